@@ -1,0 +1,139 @@
+"""ctypes binding of the CPU oracle (oracle/fe_oracle.c).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this.  It imports nothing from paper_1412_8754_b200's CUDA binding; parameters arrive
+as the plain dict made by paper_1412_8754_b200.workloads.model_params.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+
+class FeoParams(C.Structure):
+    _fields_ = [("model", C.c_int32), ("form_factor", C.c_int32), ("t", C.c_double * 4),
+                ("mu", C.c_double), ("U", C.c_double), ("eta_scale", C.c_double),
+                ("cond_mult", C.c_double), ("band_mask", C.c_int32), ("const_mode", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        dp = C.POINTER(C.c_double)
+        ip = C.POINTER(C.c_int32)
+        pp = C.POINTER(FeoParams)
+        L.feo_num_bands.argtypes = [pp]
+        L.feo_num_bands.restype = C.c_int
+        L.feo_num_threads.restype = C.c_int
+        L.feo_set_num_threads.argtypes = [C.c_int]
+        L.feo_band_energies.argtypes = [pp, C.c_double, C.c_double, dp]
+        L.feo_band_energies.restype = None
+        L.feo_eta.argtypes = [pp, C.c_double, C.c_double]
+        L.feo_eta.restype = C.c_double
+        L.feo_quasiparticle.argtypes = [C.c_double, C.c_double, C.c_double, dp, dp]
+        L.feo_quasiparticle.restype = None
+        L.feo_thermal.argtypes = [C.c_double, C.c_double]
+        L.feo_thermal.restype = C.c_double
+        L.feo_omega_column.argtypes = [pp, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
+                                       dp, C.c_int32, dp]
+        L.feo_omega_column.restype = C.c_int
+        L.feo_omega_grid.argtypes = [pp, C.c_int32, C.c_double, dp, C.c_int32, dp, C.c_int32,
+                                     dp, C.c_int32, dp]
+        L.feo_omega_grid.restype = C.c_int
+        L.feo_argmin.argtypes = [dp, dp, C.c_int32, C.c_int32, ip, dp, dp]
+        L.feo_argmin.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _params(p: dict) -> FeoParams:
+    s = FeoParams()
+    s.model, s.form_factor = p["model"], p["form_factor"]
+    for i in range(4):
+        s.t[i] = p["t"][i]
+    s.mu, s.U, s.eta_scale, s.cond_mult = p["mu"], p["U"], p["eta_scale"], p["cond_mult"]
+    s.band_mask, s.const_mode = p["band_mask"], p["const_mode"]
+    return s
+
+
+def _dptr(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def num_threads() -> int:
+    return int(lib().feo_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().feo_set_num_threads(int(n))
+
+
+def band_energies(p: dict, kx: float, ky: float) -> np.ndarray:
+    sp = _params(p)
+    out = np.zeros(2)
+    lib().feo_band_energies(C.byref(sp), kx, ky, _dptr(out))
+    return out[: (1 if p["model"] == 1 else 2)]
+
+
+def eta(p: dict, kx: float, ky: float) -> float:
+    sp = _params(p)
+    return float(lib().feo_eta(C.byref(sp), kx, ky))
+
+
+def quasiparticle(a: float, b: float, gap: float):
+    ep, em = C.c_double(), C.c_double()
+    lib().feo_quasiparticle(a, b, gap, C.byref(ep), C.byref(em))
+    return ep.value, em.value
+
+
+def thermal(x: float, T: float) -> float:
+    return float(lib().feo_thermal(x, T))
+
+
+def omega_column(p: dict, N: int, T: float, q, h: float, delta) -> np.ndarray:
+    sp = _params(p)
+    d = np.ascontiguousarray(delta, dtype=np.float64)
+    out = np.empty(d.shape[0], dtype=np.float64)
+    rc = lib().feo_omega_column(C.byref(sp), N, T, float(q[0]), float(q[1]), float(h), _dptr(d), d.shape[0],
+                                _dptr(out))
+    if rc:
+        raise ValueError(f"feo_omega_column failed: {rc}")
+    return out
+
+
+def omega_grid(p: dict, N: int, T: float, q, h, delta) -> np.ndarray:
+    """Omega[iq, ih, id] over the full grid (Algorithm 1 loop order)."""
+    sp = _params(p)
+    q = np.ascontiguousarray(q, dtype=np.float64).reshape(-1, 2)
+    h = np.ascontiguousarray(h, dtype=np.float64).reshape(-1)
+    d = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+    out = np.empty((q.shape[0], h.shape[0], d.shape[0]), dtype=np.float64)
+    rc = lib().feo_omega_grid(C.byref(sp), N, T, _dptr(q), q.shape[0], _dptr(h), h.shape[0], _dptr(d),
+                              d.shape[0], _dptr(out))
+    if rc:
+        raise ValueError(f"feo_omega_grid failed: {rc}")
+    return out
+
+
+def argmin(omega, delta):
+    """Per-(q,h) linear search over the last axis.  Returns (idx int32, delta*, omega*)."""
+    om = np.ascontiguousarray(omega, dtype=np.float64)
+    d = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+    nd = d.shape[0]
+    ncol = om.size // nd
+    idx = np.empty(ncol, dtype=np.int32)
+    ds = np.empty(ncol)
+    os_ = np.empty(ncol)
+    rc = lib().feo_argmin(_dptr(om), _dptr(d), ncol, nd, idx.ctypes.data_as(C.POINTER(C.c_int32)), _dptr(ds),
+                          _dptr(os_))
+    if rc:
+        raise ValueError(f"feo_argmin failed: {rc}")
+    shp = om.shape[:-1]
+    return idx.reshape(shp), ds.reshape(shp), os_.reshape(shp)
