@@ -1,0 +1,147 @@
+/*
+ * fe.h -- C ABI of libfe: B200-native (sm_100a) evaluation of the mean-field grand potential
+ * Omega(Delta; q, h, T) of a lattice superconductor over an N x N Brillouin-zone grid, for every
+ * point of a (q, h, Delta) parameter grid, and the per-(q, h) global-minimum search over Delta.
+ *
+ * Method: Januszewski, Ptok, Crivelli, Gardas, "GPU-based acceleration of free energy calculations
+ * in solid state physics" (arXiv 1412.8754); citations are PAPER.md:<line> of the reference text.
+ *
+ *   Omega = sum_{eps in bands} sum_{k in grid} [ f(E+) + f(E-) + C_{eps k} ] + cond_mult N^2 Delta^2 / U
+ *   f(x)  = -T ln(1 + exp(-x/T))                                              (Eq. 5)
+ *   E+-   = (a-b)/2 +- sqrt(((a+b)/2)^2 + (Delta eta_k)^2)                    (Eq. 4)
+ *   a = E_{eps,k} - mu - h (spin up),  b = E_{eps,-k+q} - mu + h (spin down)
+ *   k = 2 pi (i, j)/N, i, j = 0..N-1;  q is any real vector (need not be on the grid).
+ *
+ * Everything is fp64.  All device work is enqueued on the CUDA stream the caller passes and the
+ * calls return without synchronising (except fe_scan_host, which is the host-buffer convenience
+ * path and returns with results in host memory).  Results are deterministic: the k-sum uses a fixed
+ * k -> thread map, a fixed shuffle tree and a fixed chunk order; there are no floating-point atomics,
+ * so the same inputs give bit-identical Omega on every run.
+ *
+ * There is NO CPU fallback: without a compute-capability 10.x device fe_create fails.
+ *
+ * Thread-safety: one handle must be used by one host thread and one stream at a time; distinct
+ * handles are independent.  No function throws or aborts across this boundary.
+ */
+#ifndef FE_H_
+#define FE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes (fe_strerror gives text; for FE_ECUDA it includes the CUDA error string) ---- */
+#define FE_OK      0
+#define FE_EINVAL (-1) /* null pointer, N < 1, T <= 0 or non-finite, U <= 0, list length < 1, unknown model/mode */
+#define FE_ENOMEM (-2) /* host or device allocation failed                                                       */
+#define FE_ECUDA  (-3) /* a CUDA runtime call or kernel launch failed                                            */
+#define FE_EARCH  (-4) /* current device is not compute capability 10.x (B200)                                   */
+
+/* ---- model selectors ---- */
+#define FE_MODEL_ONE_BAND 1 /* E_k = -2 t[0] (cos kx + cos ky): nearest-neighbour square lattice (BCS use) */
+#define FE_MODEL_TWO_BAND 2 /* Raghu et al. two-orbital model, Eqs. A.1-A.4, t[0..3] = t1..t4;
+                               band 0 = E_+ (electron-like), band 1 = E_- (hole-like)             */
+#define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
+#define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
+
+/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode) ----
+ * DENSE   : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5.
+ * WINDOWED: a term whose thermal part is below half an ulp of its T=0 part (|R-|d|| >= 37 T)
+ *           adds only max(R,|d|); the decision is taken per warp.  Same sums to rounding (bit-identical
+ *           per term; only whole warps skip work).                                                        */
+#define FE_EVAL_DENSE    0
+#define FE_EVAL_WINDOWED 1
+
+typedef struct fe_handle fe_handle; /* opaque; owns device scratch (trig tables, partial sums, staging) */
+
+typedef struct {
+  int32_t model;       /* FE_MODEL_*                                                                       */
+  int32_t form_factor; /* FE_FORM_*                                                                        */
+  double  t[4];        /* hoppings; unused entries ignored                                                 */
+  double  mu;          /* chemical potential                                                               */
+  double  U;           /* pairing strength, > 0; enters only the condensation term                         */
+  double  eta_scale;   /* 1.0 for Delta_k = Delta cos kx cos ky; 4.0 reproduces eta of PAPER.md:289        */
+  double  cond_mult;   /* condensation term = cond_mult * N^2 * Delta^2 / U; Eq. 5 per band => #bands      */
+  int32_t band_mask;   /* bit e set => band e contributes (Omega = sum_eps Omega_eps)         */
+  int32_t const_mode;  /* 0: constant of Eq. 5 = sum_k xi_{eps,-k+q,dn} (what the Bogoliubov transformation
+                             of Eq. 3 gives for any q)   1: sum_k xi_{eps,k,dn} (Eq. 5 as printed; equal for
+                             on-grid q)                                                                     */
+} fe_model_params;
+
+/* Create a handle for an N x N k-grid at temperature T (k_B = 1, energies in units of |t1|).
+ * Uses the CURRENT CUDA device.  *out is set only on success.  Errors: FE_EINVAL, FE_EARCH, FE_ENOMEM, FE_ECUDA. */
+int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** out);
+
+/* Change T (> 0, finite) for subsequent calls (config 4 scans two temperatures).  Host-only, cheap. */
+int fe_set_temperature(fe_handle* h, double T);
+
+/* Select FE_EVAL_DENSE (default) or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
+int fe_set_eval_mode(fe_handle* h, int32_t mode);
+
+/* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,
+ * deterministic two-stage k-sum; Algorithm 1 lines 1-5, Algorithm 2).
+ *   q_xy  : HOST, nq pairs (qx, qy), radians.            h_list : HOST, nh Zeeman fields.
+ *   delta : HOST, nd order-parameter amplitudes (any sign; Omega is even in Delta).
+ *   omega_dev : DEVICE, nq*nh*nd doubles, index (iq*nh + ih)*nd + id (Delta fastest); caller-owned.
+ *   cuda_stream : cudaStream_t cast to void* (NULL = legacy default stream).
+ * The three host lists are copied before the call returns and may be reused immediately.
+ * Omega is extensive (sum over k and bands, not per site).  Asynchronous w.r.t. the host.          */
+int fe_omega_grid(fe_handle* h,
+                  const double* q_xy, int32_t nq,
+                  const double* h_list, int32_t nh,
+                  const double* delta, int32_t nd,
+                  double* omega_dev, void* cuda_stream);
+
+/* Per-(q, h) global minimum over Delta (Algorithm 1 line 6; step 3 of PAPER.md:169, moved on-device).
+ *   omega_dev : DEVICE, ncol*nd doubles, Delta fastest (the layout fe_omega_grid writes; ncol = nq*nh).
+ *   delta     : HOST, nd values (copied before return).
+ *   idx_dev (int32), delta_star_dev, omega_star_dev : DEVICE, ncol each; any of them may be NULL.
+ * Lowest Omega wins; among exactly equal values the lowest index wins.  NaN never wins.             */
+int fe_argmin(fe_handle* h, const double* omega_dev, const double* delta,
+              int32_t ncol, int32_t nd,
+              int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev, void* cuda_stream);
+
+/* Host-buffer end-to-end path: copies the lists to the device, runs fe_omega_grid and fe_argmin,
+ * copies results back and SYNCHRONISES the stream.  All pointers are HOST memory (pinned or pageable).
+ *   omega_host : nq*nh*nd doubles or NULL (skip the Omega copy-back);
+ *   idx_host / delta_star_host / omega_star_host : nq*nh each, any may be NULL.                     */
+int fe_scan_host(fe_handle* h,
+                 const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                 const double* delta, int32_t nd,
+                 double* omega_host, int32_t* idx_host, double* delta_star_host, double* omega_star_host,
+                 void* cuda_stream);
+
+/* Kernel timing for roofline reports.  When enabled, fe_omega_grid brackets its k-sum kernel (K1) with
+ * CUDA events on the launching stream; after the caller has synchronised the stream, fe_get_timing returns
+ * the duration of the most recent K1 launch (ms) and the number of (k, band, q, h, Delta) terms it evaluated. */
+int fe_enable_timing(fe_handle* h, int32_t on);
+int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
+
+/* Number of kernel launches this handle has issued since creation (all kernels of this library). */
+int fe_get_launch_count(fe_handle* h, int64_t* launches);
+
+/* Tuning knobs (optional).  tile: 0 = auto, else index into the built-in tile table (see fe_tile_info);
+ * target_blocks: minimum number of thread blocks K1 should be split into (0 = auto).               */
+int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks);
+int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past the end of the table */
+
+/* FP64 DFMA-chain microbenchmark on the current device (register-resident, no memory traffic):
+ * runs `blocks` blocks of 256 threads, each thread `iters` x 16 dependent-chain-interleaved DFMAs,
+ * and returns elapsed ms and the number of DFMA instructions (thread-level) executed.
+ * Used to measure the FP64 roofline denominator in the same run as the benchmark.                  */
+int fe_fp64_peak_probe(int32_t blocks, int32_t iters, float* ms, double* dfma_count, void* cuda_stream);
+
+/* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
+ * y[i] = exp(x[i]) for x <= 0 (which = 0) or ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the k-sum
+ * kernel evaluates the thermal term of Eq. 5.  Lets tests check it in isolation.       */
+int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream);
+
+void fe_destroy(fe_handle* h);          /* frees all device/host scratch; NULL is a no-op */
+const char* fe_strerror(int code);      /* static or thread-local string; never NULL      */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FE_H_ */

@@ -1,0 +1,526 @@
+// fe_api.cu -- C ABI of libfe (include/fe.h): handle, validation, launch logic.  No torch types, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/fe.h"
+#include "fe_kernels.cuh"
+
+namespace {
+
+using namespace fe;
+
+thread_local char g_errbuf[512] = "no error";
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_errbuf, sizeof g_errbuf, "CUDA error in %s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+  return FE_ECUDA;
+}
+#define FE_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+struct Tile { int th, td; };
+constexpr Tile kTiles[] = {{8, 4}, {4, 4}, {2, 8}, {1, 8}};
+constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
+constexpr int kStageSlots = 4;
+constexpr int kSChunksMax = 128;
+
+struct StageSlot {
+  double* host = nullptr;    // pinned
+  double* dev = nullptr;
+  size_t cap = 0;            // doubles
+  cudaEvent_t ev = nullptr;  // recorded after the H2D copy out of `host`
+  bool pending = false;
+};
+
+}  // namespace
+
+struct fe_handle {
+  fe_model_params p;
+  int32_t N = 0;
+  double T = 0;
+  int32_t mode = FE_EVAL_DENSE;
+  int32_t tile = 0;            // 0 = auto, else 1 + index
+  int32_t target_blocks = 0;   // 0 = auto
+  int device = 0;
+  int sm_count = 148;
+  int nb = 1;
+  // device scratch
+  MathTabs* d_tabs = nullptr;
+  double4* d_coltab = nullptr;
+  double4* d_rowtab = nullptr;
+  size_t coltab_cap = 0, rowtab_cap = 0;
+  double* d_partial = nullptr;
+  size_t partial_cap = 0;
+  double* d_spart = nullptr;
+  size_t spart_cap = 0;
+  double* d_omega = nullptr;   // fe_scan_host only
+  size_t omega_cap = 0;
+  void* d_res = nullptr;       // fe_scan_host: idx | dstar | ostar
+  size_t res_cap = 0;          // columns
+  StageSlot slots[kStageSlots];
+  int next_slot = 0;
+  // timing
+  bool timing = false;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timing_valid = false;
+  double last_band_evals = 0;
+  int64_t launches = 0;
+};
+
+namespace {
+
+int nbands(const fe_model_params& p) { return p.model == FE_MODEL_ONE_BAND ? 1 : 2; }
+
+bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
+
+int validate_params(const fe_model_params* p, int32_t N, double T) {
+  if (!p) { snprintf(g_errbuf, sizeof g_errbuf, "params is NULL"); return FE_EINVAL; }
+  if (p->model != FE_MODEL_ONE_BAND && p->model != FE_MODEL_TWO_BAND) {
+    snprintf(g_errbuf, sizeof g_errbuf, "unknown model %d", p->model); return FE_EINVAL; }
+  if (p->form_factor != FE_FORM_S && p->form_factor != FE_FORM_SPM) {
+    snprintf(g_errbuf, sizeof g_errbuf, "unknown form_factor %d", p->form_factor); return FE_EINVAL; }
+  if (p->const_mode != 0 && p->const_mode != 1) {
+    snprintf(g_errbuf, sizeof g_errbuf, "const_mode must be 0 or 1"); return FE_EINVAL; }
+  if (N < 1 || N > 65536) { snprintf(g_errbuf, sizeof g_errbuf, "N must be in [1, 65536]"); return FE_EINVAL; }
+  if (!finite_pos(T)) { snprintf(g_errbuf, sizeof g_errbuf, "T must be finite and > 0"); return FE_EINVAL; }
+  if (!finite_pos(p->U)) { snprintf(g_errbuf, sizeof g_errbuf, "U must be finite and > 0"); return FE_EINVAL; }
+  const int nb = nbands(*p);
+  for (int i = 0; i < (nb == 1 ? 1 : 4); ++i)
+    if (!isfinite(p->t[i])) { snprintf(g_errbuf, sizeof g_errbuf, "t[%d] is not finite", i); return FE_EINVAL; }
+  if (!isfinite(p->mu) || !isfinite(p->eta_scale) || !isfinite(p->cond_mult)) {
+    snprintf(g_errbuf, sizeof g_errbuf, "mu, eta_scale, cond_mult must be finite"); return FE_EINVAL; }
+  if (p->band_mask < 0 || p->band_mask >= (1 << nb)) {
+    snprintf(g_errbuf, sizeof g_errbuf, "band_mask out of range for %d band(s)", nb); return FE_EINVAL; }
+  return FE_OK;
+}
+
+void build_tabs(MathTabs* t) {
+  for (int j = 0; j < kExpTabN; ++j) t->exp2_j64[j] = (double)exp2l((long double)j / 64.0L);
+  for (int idx = 0; idx < kLogTabN; ++idx) {
+    const int e = idx >> 7, i = idx & 127;
+    const long double c = ldexpl(1.0L + ((long double)i + 0.5L) / 128.0L, e);
+    const double inv = (double)(1.0L / c);
+    t->log_tab[idx].x = inv;
+    t->log_tab[idx].y = (double)(-logl((long double)inv));   // ln of the centre actually used (1/inv), not of c
+  }
+}
+
+ModelConsts make_consts(const fe_model_params& p) {
+  ModelConsts mc;
+  if (p.model == FE_MODEL_ONE_BAND) {
+    mc.tp = -2.0 * p.t[0]; mc.tm = 0; mc.t3x4 = 0; mc.t4x4 = 0;
+  } else {
+    mc.tp = -(p.t[0] + p.t[1]);
+    mc.tm = -(p.t[0] - p.t[1]);
+    mc.t3x4 = -4.0 * p.t[2];
+    mc.t4x4 = -4.0 * p.t[3];
+  }
+  mc.mu = p.mu; mc.eta_scale = p.eta_scale; mc.band_mask = p.band_mask; mc.const_mode = p.const_mode;
+  return mc;
+}
+
+template <typename T>
+int ensure(T*& ptr, size_t& cap, size_t need) {
+  if (need <= cap && ptr) return FE_OK;
+  if (ptr) { cudaFree(ptr); ptr = nullptr; cap = 0; }
+  // grow geometrically to avoid reallocation on slowly growing grids
+  size_t want = need + need / 4;
+  cudaError_t e = cudaMalloc((void**)&ptr, want * sizeof(T));
+  if (e != cudaSuccess) {
+    e = cudaMalloc((void**)&ptr, need * sizeof(T));
+    want = need;
+  }
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    snprintf(g_errbuf, sizeof g_errbuf, "device allocation of %zu bytes failed", need * sizeof(T));
+    ptr = nullptr;
+    return FE_ENOMEM;
+  }
+  cap = want;
+  return FE_OK;
+}
+
+// Copy `n` doubles assembled by `fill` into a pinned slot and enqueue the H2D copy.  Returns the device pointer.
+int stage_lists(fe_handle* h, size_t n, cudaStream_t st, double** host_out, double** dev_out, StageSlot** slot_out) {
+  StageSlot& s = h->slots[h->next_slot];
+  h->next_slot = (h->next_slot + 1) % kStageSlots;
+  if (s.pending) { FE_CUDA(cudaEventSynchronize(s.ev)); s.pending = false; }
+  if (n > s.cap) {
+    if (s.host) cudaFreeHost(s.host);
+    if (s.dev) cudaFree(s.dev);
+    s.host = nullptr; s.dev = nullptr; s.cap = 0;
+    const size_t want = n + 256;
+    if (cudaMallocHost((void**)&s.host, want * sizeof(double)) != cudaSuccess ||
+        cudaMalloc((void**)&s.dev, want * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      snprintf(g_errbuf, sizeof g_errbuf, "staging allocation of %zu doubles failed", want);
+      return FE_ENOMEM;
+    }
+    s.cap = want;
+  }
+  if (!s.ev) FE_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+  (void)st;
+  *host_out = s.host; *dev_out = s.dev; *slot_out = &s;
+  return FE_OK;
+}
+
+int choose_tile(const fe_handle* h, int nh, int nd) {
+  if (h->tile > 0) return h->tile - 1;
+  // least padded work; ties go to the earlier (larger / better amortised) tile
+  int best = 0; double best_cost = 1e300;
+  for (int t = 0; t < kNumTiles; ++t) {
+    const double padded = (double)((nh + kTiles[t].th - 1) / kTiles[t].th * kTiles[t].th) *
+                          (double)((nd + kTiles[t].td - 1) / kTiles[t].td * kTiles[t].td);
+    // sqrt + dispersion overhead per evaluation shrinks with TH: mild preference for tall tiles
+    const double cost = padded * (1.0 + 0.28 / kTiles[t].th);
+    if (cost < best_cost * (1.0 - 1e-12)) { best_cost = cost; best = t; }
+  }
+  return best;
+}
+
+template <int NB, int FORM, int TH, int TD>
+cudaError_t launch_ksum_mode(int mode, int grid, cudaStream_t st, const KsumParams& P) {
+  if (mode == FE_EVAL_WINDOWED) fe_ksum_kernel<NB, FORM, TH, TD, 1><<<grid, kThreads, 0, st>>>(P);
+  else                          fe_ksum_kernel<NB, FORM, TH, TD, 0><<<grid, kThreads, 0, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int TH, int TD>
+cudaError_t launch_ksum_tile(int nb, int form, int mode, int grid, cudaStream_t st, const KsumParams& P) {
+  if (nb == 1) return form == 0 ? launch_ksum_mode<1, 0, TH, TD>(mode, grid, st, P)
+                                : launch_ksum_mode<1, 1, TH, TD>(mode, grid, st, P);
+  return form == 0 ? launch_ksum_mode<2, 0, TH, TD>(mode, grid, st, P)
+                   : launch_ksum_mode<2, 1, TH, TD>(mode, grid, st, P);
+}
+
+cudaError_t launch_ksum(int tile, int nb, int form, int mode, int grid, cudaStream_t st, const KsumParams& P) {
+  switch (tile) {
+    case 0: return launch_ksum_tile<8, 4>(nb, form, mode, grid, st, P);
+    case 1: return launch_ksum_tile<4, 4>(nb, form, mode, grid, st, P);
+    case 2: return launch_ksum_tile<2, 8>(nb, form, mode, grid, st, P);
+    default: return launch_ksum_tile<1, 8>(nb, form, mode, grid, st, P);
+  }
+}
+
+int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh, const double* delta, int32_t nd) {
+  if (!q_xy || !h_list || !delta) { snprintf(g_errbuf, sizeof g_errbuf, "a list pointer is NULL"); return FE_EINVAL; }
+  if (nq < 1 || nh < 1 || nd < 1) { snprintf(g_errbuf, sizeof g_errbuf, "nq, nh, nd must be >= 1"); return FE_EINVAL; }
+  if ((double)nq * nh * nd > 2.0e9) { snprintf(g_errbuf, sizeof g_errbuf, "grid too large (nq*nh*nd > 2e9)"); return FE_EINVAL; }
+  for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
+  for (int i = 0; i < nh; ++i) if (!isfinite(h_list[i])) { snprintf(g_errbuf, sizeof g_errbuf, "h[%d] not finite", i); return FE_EINVAL; }
+  for (int i = 0; i < nd; ++i) if (!isfinite(delta[i])) { snprintf(g_errbuf, sizeof g_errbuf, "delta[%d] not finite", i); return FE_EINVAL; }
+  return FE_OK;
+}
+
+int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                    const double* delta, int32_t nd, double* omega_dev, cudaStream_t st) {
+  const int N = h->N;
+  // ---- stage lists: [q (2nq) | h (nh) | delta^2 (nd)] ----
+  const size_t nlist = (size_t)2 * nq + nh + nd;
+  double *hs, *ds; StageSlot* slot;
+  int rc = stage_lists(h, nlist, st, &hs, &ds, &slot);
+  if (rc) return rc;
+  memcpy(hs, q_xy, sizeof(double) * 2 * nq);
+  memcpy(hs + 2 * nq, h_list, sizeof(double) * nh);
+  for (int i = 0; i < nd; ++i) hs[2 * nq + nh + i] = delta[i] * delta[i];
+  FE_CUDA(cudaMemcpyAsync(ds, hs, nlist * sizeof(double), cudaMemcpyHostToDevice, st));
+  FE_CUDA(cudaEventRecord(slot->ev, st));
+  slot->pending = true;
+  const double* d_q = ds;
+  const double* d_h = ds + 2 * nq;
+  const double* d_d2 = ds + 2 * nq + nh;
+
+  // ---- geometry ----
+  const int tile = choose_tile(h, nh, nd);
+  const int TH = kTiles[tile].th, TD = kTiles[tile].td;
+  KsumParams P;
+  P.mc = make_consts(h->p);
+  P.T = h->T; P.neg_beta = -1.0 / h->T; P.window = 37.0 * h->T;
+  P.N = N; P.nq = nq; P.nh = nh; P.nd = nd;
+  P.ntile_h = (nh + TH - 1) / TH;
+  P.ntile_d = (nd + TD - 1) / TD;
+  int bxl = 8;                                   // 256 columns per block when N allows it
+  while (bxl > 5 && (1 << (bxl - 1)) >= N) --bxl;
+  P.bx_log2 = bxl;
+  const int bx = 1 << bxl, by = kThreads >> bxl;
+  P.ncg = (N + bx - 1) / bx;
+  const long long ntiles = (long long)nq * P.ntile_h * P.ntile_d;
+  const long long target = h->target_blocks > 0 ? h->target_blocks : (long long)h->sm_count * 2 * 24;
+  long long nrs = (target + ntiles * P.ncg - 1) / (ntiles * P.ncg);
+  const int max_nrs = (N + by - 1) / by;         // at least one row per row lane
+  if (nrs > max_nrs) nrs = max_nrs;
+  if (nrs < 1) nrs = 1;
+  int rpc = (int)((N + nrs - 1) / nrs);
+  rpc = (rpc + by - 1) / by * by;                // whole row-lane strides per chunk
+  P.rows_per_chunk = rpc;
+  P.nrs = (N + rpc - 1) / rpc;
+  P.ksplit = P.ncg * P.nrs;
+  const long long grid_ll = ntiles * P.ksplit;
+  if (grid_ll > 2147483647LL) { snprintf(g_errbuf, sizeof g_errbuf, "grid too large"); return FE_EINVAL; }
+
+  const size_t nout = (size_t)nq * nh * nd;
+  if ((rc = ensure(h->d_coltab, h->coltab_cap, (size_t)nq * N))) return rc;
+  if ((rc = ensure(h->d_rowtab, h->rowtab_cap, (size_t)nq * N))) return rc;
+  if ((rc = ensure(h->d_partial, h->partial_cap, (size_t)P.ksplit * nout))) return rc;
+  int nschunk = N < kSChunksMax ? N : kSChunksMax;
+  const int srpc = (N + nschunk - 1) / nschunk;
+  nschunk = (N + srpc - 1) / srpc;
+  if ((rc = ensure(h->d_spart, h->spart_cap, (size_t)nq * nschunk))) return rc;
+
+  P.coltab = h->d_coltab; P.rowtab = h->d_rowtab; P.h = d_h; P.d2 = d_d2; P.tabs = h->d_tabs;
+  P.partial = h->d_partial;
+
+  // ---- K0 trig, KS constant sum, K1 k-sum, K2 finish ----
+  {
+    const int n = N * nq;
+    fe_trig_kernel<<<(n + 255) / 256, 256, 0, st>>>(N, nq, d_q, h->d_coltab, h->d_rowtab);
+    FE_CUDA(cudaGetLastError());
+    h->launches++;
+  }
+  {
+    dim3 g(nschunk, nq);
+    if (h->nb == 1) fe_ssum_kernel<1><<<g, kThreads, 0, st>>>(P.mc, N, srpc, h->d_coltab, h->d_rowtab, h->d_spart);
+    else            fe_ssum_kernel<2><<<g, kThreads, 0, st>>>(P.mc, N, srpc, h->d_coltab, h->d_rowtab, h->d_spart);
+    FE_CUDA(cudaGetLastError());
+    h->launches++;
+  }
+  if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
+  FE_CUDA(launch_ksum(tile, h->nb, h->p.form_factor, h->mode, (int)grid_ll, st, P));
+  h->launches++;
+  if (h->timing) {
+    FE_CUDA(cudaEventRecord(h->ev1, st));
+    h->timing_valid = true;
+    int nbm = 0;
+    for (int e = 0; e < h->nb; ++e) nbm += (h->p.band_mask >> e) & 1;
+    h->last_band_evals = (double)N * N * nbm * (double)nout;
+  }
+  {
+    const double condc = h->p.cond_mult * (double)N * (double)N / h->p.U;
+    fe_finish_kernel<<<(unsigned)((nout + 255) / 256), 256, 0, st>>>(nq, nh, nd, P.ksplit, nschunk, condc,
+                                                                      h->d_partial, h->d_spart, d_d2, omega_dev);
+    FE_CUDA(cudaGetLastError());
+    h->launches++;
+  }
+  return FE_OK;
+}
+
+int argmin_impl(fe_handle* h, const double* omega_dev, const double* delta, int32_t ncol, int32_t nd,
+                int32_t* idx_dev, double* dstar_dev, double* ostar_dev, cudaStream_t st) {
+  double *hs, *ds; StageSlot* slot;
+  int rc = stage_lists(h, (size_t)nd, st, &hs, &ds, &slot);
+  if (rc) return rc;
+  memcpy(hs, delta, sizeof(double) * nd);
+  FE_CUDA(cudaMemcpyAsync(ds, hs, (size_t)nd * sizeof(double), cudaMemcpyHostToDevice, st));
+  FE_CUDA(cudaEventRecord(slot->ev, st));
+  slot->pending = true;
+  const int wpb = 8;
+  fe_argmin_kernel<<<(ncol + wpb - 1) / wpb, wpb * 32, 0, st>>>(ncol, nd, omega_dev, ds, idx_dev, dstar_dev, ostar_dev);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  return FE_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+// C ABI
+// =====================================================================================================
+extern "C" {
+
+int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** out) {
+  if (!out) { snprintf(g_errbuf, sizeof g_errbuf, "out is NULL"); return FE_EINVAL; }
+  int rc = validate_params(params, N, T);
+  if (rc) return rc;
+  int dev = 0;
+  FE_CUDA(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  FE_CUDA(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) {
+    snprintf(g_errbuf, sizeof g_errbuf, "device %d (%s) is compute capability %d.%d; libfe is built for sm_100a only",
+             dev, prop.name, prop.major, prop.minor);
+    return FE_EARCH;
+  }
+  fe_handle* h = new (std::nothrow) fe_handle();
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "host allocation failed"); return FE_ENOMEM; }
+  h->p = *params; h->N = N; h->T = T; h->device = dev; h->sm_count = prop.multiProcessorCount;
+  h->nb = nbands(*params);
+  MathTabs host_tabs;
+  memset(&host_tabs, 0, sizeof host_tabs);
+  build_tabs(&host_tabs);
+  cudaError_t e = cudaMalloc((void**)&h->d_tabs, sizeof(MathTabs));
+  if (e == cudaSuccess) e = cudaMemcpy(h->d_tabs, &host_tabs, sizeof(MathTabs), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaEventCreate(&h->ev0);
+  if (e == cudaSuccess) e = cudaEventCreate(&h->ev1);
+  if (e != cudaSuccess) { rc = cuda_fail(e, "fe_create setup"); fe_destroy(h); return rc; }
+  *out = h;
+  return FE_OK;
+}
+
+int fe_set_temperature(fe_handle* h, double T) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (!finite_pos(T)) { snprintf(g_errbuf, sizeof g_errbuf, "T must be finite and > 0"); return FE_EINVAL; }
+  h->T = T;
+  return FE_OK;
+}
+
+int fe_set_eval_mode(fe_handle* h, int32_t mode) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (mode != FE_EVAL_DENSE && mode != FE_EVAL_WINDOWED) {
+    snprintf(g_errbuf, sizeof g_errbuf, "unknown eval mode %d", mode); return FE_EINVAL; }
+  h->mode = mode;
+  return FE_OK;
+}
+
+int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (tile < 0 || tile > kNumTiles || target_blocks < 0) {
+    snprintf(g_errbuf, sizeof g_errbuf, "tile must be in [0, %d], target_blocks >= 0", kNumTiles); return FE_EINVAL; }
+  h->tile = tile; h->target_blocks = target_blocks;
+  return FE_OK;
+}
+
+int fe_tile_info(int32_t tile, int32_t* th, int32_t* td) {
+  if (tile < 1 || tile > kNumTiles) { snprintf(g_errbuf, sizeof g_errbuf, "no such tile"); return FE_EINVAL; }
+  if (th) *th = kTiles[tile - 1].th;
+  if (td) *td = kTiles[tile - 1].td;
+  return FE_OK;
+}
+
+int fe_omega_grid(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                  const double* delta, int32_t nd, double* omega_dev, void* cuda_stream) {
+  if (!h || !omega_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle or omega_dev is NULL"); return FE_EINVAL; }
+  int rc = check_lists(q_xy, nq, h_list, nh, delta, nd);
+  if (rc) return rc;
+  return omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, omega_dev, (cudaStream_t)cuda_stream);
+}
+
+int fe_argmin(fe_handle* h, const double* omega_dev, const double* delta, int32_t ncol, int32_t nd,
+              int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev, void* cuda_stream) {
+  if (!h || !omega_dev || !delta) { snprintf(g_errbuf, sizeof g_errbuf, "handle, omega_dev or delta is NULL"); return FE_EINVAL; }
+  if (ncol < 1 || nd < 1) { snprintf(g_errbuf, sizeof g_errbuf, "ncol, nd must be >= 1"); return FE_EINVAL; }
+  return argmin_impl(h, omega_dev, delta, ncol, nd, idx_dev, delta_star_dev, omega_star_dev, (cudaStream_t)cuda_stream);
+}
+
+int fe_scan_host(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                 const double* delta, int32_t nd, double* omega_host, int32_t* idx_host,
+                 double* delta_star_host, double* omega_star_host, void* cuda_stream) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  int rc = check_lists(q_xy, nq, h_list, nh, delta, nd);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nout = (size_t)nq * nh * nd;
+  const size_t ncol = (size_t)nq * nh;
+  if ((rc = ensure(h->d_omega, h->omega_cap, nout))) return rc;
+  {
+    char* p = (char*)h->d_res;
+    size_t cap = h->res_cap;
+    if (ncol > cap || !p) {
+      if (p) cudaFree(p);
+      h->d_res = nullptr; h->res_cap = 0;
+      if (cudaMalloc(&h->d_res, ncol * 24) != cudaSuccess) {
+        cudaGetLastError(); snprintf(g_errbuf, sizeof g_errbuf, "device allocation failed"); return FE_ENOMEM; }
+      h->res_cap = ncol;
+    }
+  }
+  double* d_dstar = (double*)h->d_res;
+  double* d_ostar = d_dstar + h->res_cap;
+  int32_t* d_idx = (int32_t*)(d_ostar + h->res_cap);
+  if ((rc = omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, h->d_omega, st))) return rc;
+  if ((rc = argmin_impl(h, h->d_omega, delta, (int32_t)ncol, nd, d_idx, d_dstar, d_ostar, st))) return rc;
+  if (omega_host) FE_CUDA(cudaMemcpyAsync(omega_host, h->d_omega, nout * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (idx_host) FE_CUDA(cudaMemcpyAsync(idx_host, d_idx, ncol * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (delta_star_host) FE_CUDA(cudaMemcpyAsync(delta_star_host, d_dstar, ncol * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (omega_star_host) FE_CUDA(cudaMemcpyAsync(omega_star_host, d_ostar, ncol * sizeof(double), cudaMemcpyDeviceToHost, st));
+  FE_CUDA(cudaStreamSynchronize(st));
+  return FE_OK;
+}
+
+int fe_enable_timing(fe_handle* h, int32_t on) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  h->timing = on != 0;
+  h->timing_valid = false;
+  return FE_OK;
+}
+
+int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (!h->timing_valid) { snprintf(g_errbuf, sizeof g_errbuf, "no timed launch recorded"); return FE_EINVAL; }
+  float ms = 0;
+  FE_CUDA(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+  if (ksum_ms) *ksum_ms = ms;
+  if (band_evals) *band_evals = h->last_band_evals;
+  return FE_OK;
+}
+
+int fe_get_launch_count(fe_handle* h, int64_t* launches) {
+  if (!h || !launches) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+  *launches = h->launches;
+  return FE_OK;
+}
+
+int fe_fp64_peak_probe(int32_t blocks, int32_t iters, float* ms, double* dfma_count, void* cuda_stream) {
+  if (blocks < 1 || iters < 1 || !ms || !dfma_count) { snprintf(g_errbuf, sizeof g_errbuf, "bad argument"); return FE_EINVAL; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  double* sink = nullptr;
+  cudaEvent_t a = nullptr, b = nullptr;
+  FE_CUDA(cudaMalloc((void**)&sink, sizeof(double)));
+  cudaError_t e = cudaEventCreate(&a);
+  if (e == cudaSuccess) e = cudaEventCreate(&b);
+  if (e == cudaSuccess) { fe_dfma_probe_kernel<<<blocks, 256, 0, st>>>(16, 1.0, sink); e = cudaGetLastError(); }  // warm-up
+  if (e == cudaSuccess) e = cudaEventRecord(a, st);
+  if (e == cudaSuccess) { fe_dfma_probe_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, sink); e = cudaGetLastError(); }
+  if (e == cudaSuccess) e = cudaEventRecord(b, st);
+  if (e == cudaSuccess) e = cudaEventSynchronize(b);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms, a, b);
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
+  cudaFree(sink);
+  if (e != cudaSuccess) return cuda_fail(e, "fe_fp64_peak_probe");
+  *dfma_count = (double)blocks * 256.0 * (double)iters * 16.0;
+  return FE_OK;
+}
+
+// Diagnostic entry used by the GPU tests: y[i] = exp_nonpos(x[i]) (which = 0) or log_1p_w(x[i]) (which = 1).
+// x_dev, y_dev: DEVICE arrays of n doubles.  Not part of the method; exported so the device math can be
+// checked in isolation against numpy.
+int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream) {
+  if (!h || !x_dev || !y_dev || n < 1 || (which != 0 && which != 1)) { snprintf(g_errbuf, sizeof g_errbuf, "bad argument"); return FE_EINVAL; }
+  fe_math_probe_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(which, n, x_dev, y_dev, h->d_tabs);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  return FE_OK;
+}
+
+void fe_destroy(fe_handle* h) {
+  if (!h) return;
+  cudaFree(h->d_tabs); cudaFree(h->d_coltab); cudaFree(h->d_rowtab); cudaFree(h->d_partial);
+  cudaFree(h->d_spart); cudaFree(h->d_omega); cudaFree(h->d_res);
+  for (auto& s : h->slots) {
+    if (s.pending && s.ev) cudaEventSynchronize(s.ev);
+    if (s.host) cudaFreeHost(s.host);
+    if (s.dev) cudaFree(s.dev);
+    if (s.ev) cudaEventDestroy(s.ev);
+  }
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+  cudaGetLastError();
+  delete h;
+}
+
+const char* fe_strerror(int code) {
+  switch (code) {
+    case FE_OK: return "ok";
+    case FE_EINVAL: case FE_ENOMEM: case FE_ECUDA: case FE_EARCH: return g_errbuf;
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

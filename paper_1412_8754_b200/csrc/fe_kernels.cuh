@@ -1,0 +1,348 @@
+// fe_kernels.cuh -- sm_100a kernels of the Omega(Delta; q, h, T) hot path.
+//
+//   K0  fe_trig_kernel    cos/sin of the N grid angles and of the N shifted angles k - q, per q      (S1)
+//   KS  fe_ssum_kernel    S[q] = sum_{k,band} s_k  (the h- and Delta-independent part of Eq. 5)      (S2, S3, S8)
+//   K1  fe_ksum_kernel    P[chunk][q,h,Delta] = sum_{k in chunk, band} (max(R,|d|) + T ln(1+w))      (S2-S6, S8)
+//   K2  fe_finish_kernel  Omega = S[q] - sum_chunk P + cond_mult N^2 Delta^2/U, fixed chunk order    (S7, S9)
+//   K3  fe_argmin_kernel  per-(q,h) lowest Omega over Delta, lowest index on ties                    (S10)
+//
+// Algebra (PAPER.md:89 Eq. 4, :94 Eq. 5; derivation in DESIGN.md): with a = xi_up(k), b = xi_dn(-k+q),
+// s = (a+b)/2, d = (a-b)/2 = d0 - h, R = sqrt(s^2 + Delta^2 eta_k^2):
+//     f(d+R) + f(d-R) + b = s - max(R,|d|) - T ln(1 + u + v + u v),  u = e^{-|R-|d||/T}, v = e^{-(R+|d|)/T}.
+// s, R do not depend on h; d does not depend on Delta: a thread keeps a TH x TD register tile of (h, Delta)
+// accumulators, computes TD square roots and TH field shifts per (k, band), and reuses the dispersion for all.
+// k-points are generated in registers (a thread owns one kx column and walks ky rows); nothing but the
+// few-KB trig tables and parameter lists is read from memory.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fe_math.cuh"
+
+namespace fe {
+
+constexpr int kThreads = 256;          // threads per K1 / KS block
+constexpr int kWarps = kThreads / 32;
+
+struct ModelConsts {                   // host-precomputed combinations of the hoppings (A.1-A.4)
+  double tp;                           // two-band: -(t1 + t2)         one-band: -2 t
+  double tm;                           // two-band: -(t1 - t2)
+  double t3x4;                         // -4 t3
+  double t4x4;                         // -4 t4
+  double mu;
+  double eta_scale;
+  int32_t band_mask;
+  int32_t const_mode;
+};
+
+struct KsumParams {
+  ModelConsts mc;
+  double T, neg_beta, window;          // window = 37 T (FE_EVAL_WINDOWED threshold on |R - |d||)
+  int32_t N, nq, nh, nd;
+  int32_t ntile_h, ntile_d;
+  int32_t bx_log2;                     // block = 2^bx_log2 columns x (256 >> bx_log2) row lanes
+  int32_t ncg, nrs, rows_per_chunk, ksplit;   // column groups, row splits; ksplit = ncg * nrs
+  const double4* coltab;               // [nq][N] {cos kx, sin kx, cos(kx-qx), sin(kx-qx)}
+  const double4* rowtab;               // [nq][N] {cos ky, sin ky, cos(ky-qy), sin(ky-qy)}
+  const double* h;                     // [nh]
+  const double* d2;                    // [nd]  Delta^2
+  const MathTabs* tabs;                // global copy of the exp/log tables
+  double* partial;                     // [ksplit][nq*nh*nd]
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Band energies at one k from its four trig values (S2).  E[0] = E_+, E[1] = E_- (A.4).
+// ---------------------------------------------------------------------------------------------------
+template <int NB>
+__device__ __forceinline__ void band_energies(const ModelConsts& mc, double cx, double sx, double cy, double sy,
+                                              double (&E)[NB]) {
+  if (NB == 1) {
+    E[0] = mc.tp * (cx + cy);
+  } else {
+    // (T11+T22)/2 = -(t1+t2)(cx+cy) - 4 t3 cx cy ; (T11-T22)/2 = -(t1-t2)(cx-cy) ; T12 = -4 t4 sx sy
+    const double avg = fma(mc.t3x4, cx * cy, mc.tp * (cx + cy));
+    const double dif = mc.tm * (cx - cy);
+    const double off = mc.t4x4 * (sx * sy);
+    const double rad = sqrt(fma(dif, dif, off * off));
+    E[0] = avg + rad;
+    E[NB - 1] = avg - rad;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// K0: trig tables.  One thread per (iq, i).  Angles are formed exactly as k = 2 pi i / N and k - q in fp64
+// and evaluated with CUDA's sincos (<= 2 ulp); E is even, so E(-k+q) = E(k-q).
+// ---------------------------------------------------------------------------------------------------
+__global__ void fe_trig_kernel(int N, int nq, const double* __restrict__ q_xy, double4* __restrict__ coltab,
+                               double4* __restrict__ rowtab) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * nq) return;
+  const int iq = idx / N, i = idx - iq * N;
+  const double k = 2.0 * 3.14159265358979323846 * (double)i / (double)N;
+  double s0, c0, s1, c1;
+  sincos(k, &s0, &c0);
+  sincos(k - q_xy[2 * iq], &s1, &c1);
+  coltab[idx] = make_double4(c0, s0, c1, s1);
+  sincos(k - q_xy[2 * iq + 1], &s1, &c1);
+  rowtab[idx] = make_double4(c0, s0, c1, s1);
+}
+
+// Fixed-order block sum of one double per thread; result valid in thread 0.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// KS: spart[iq][chunk] = sum over the chunk's rows, all columns, masked bands of  s  (+ 2 d0 if const_mode 1).
+// Kahan-compensated per thread (it is cheap here), then a fixed tree.  grid = (nchunk, nq).
+// ---------------------------------------------------------------------------------------------------
+template <int NB>
+__global__ void __launch_bounds__(kThreads) fe_ssum_kernel(ModelConsts mc, int N, int rows_per_chunk,
+                                                           const double4* __restrict__ coltab,
+                                                           const double4* __restrict__ rowtab,
+                                                           double* __restrict__ spart) {
+  const int iq = blockIdx.y, chunk = blockIdx.x;
+  const int r0 = chunk * rows_per_chunk;
+  const int r1 = min(N, r0 + rows_per_chunk);
+  const double4* ct = coltab + (size_t)iq * N;
+  const double4* rt = rowtab + (size_t)iq * N;
+  double sum = 0.0, comp = 0.0;
+  const int total = (r1 > r0 ? (r1 - r0) : 0) * N;
+  for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+    const int r = r0 + idx / N, c = idx % N;
+    const double4 cc = ct[c], rr = rt[r];
+    double Ek[NB], Eq[NB];
+    band_energies<NB>(mc, cc.x, cc.y, rr.x, rr.y, Ek);
+    band_energies<NB>(mc, cc.z, cc.w, rr.z, rr.w, Eq);
+#pragma unroll
+    for (int e = 0; e < NB; ++e) {
+      if (!((mc.band_mask >> e) & 1)) continue;
+      double term = fma(0.5, Ek[e] + Eq[e], -mc.mu);          // s
+      if (mc.const_mode == 1) term += Ek[e] - Eq[e];         // + 2 d0  (Eq. 5 literal constant)
+      const double y = term - comp;
+      const double t = sum + y;
+      comp = (t - sum) - y;
+      sum = t;
+    }
+  }
+  __shared__ double red[kWarps];
+  double w = warp_sum(sum);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = w;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+#pragma unroll
+    for (int i = 0; i < kWarps; ++i) tot += red[i];
+    spart[(size_t)iq * gridDim.x + chunk] = tot;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// K1: the k-sum.  Block = (iq, h-tile, Delta-tile, k-chunk).  Thread = one kx column x a strided set of ky rows.
+// ---------------------------------------------------------------------------------------------------
+template <int NB, int FORM, int TH, int TD, int MODE>
+__global__ void __launch_bounds__(kThreads) fe_ksum_kernel(const KsumParams P) {
+  __shared__ MathTabs tabs;
+  __shared__ double red[kWarps][TH * TD];
+
+  // stage the exp/log tables (4.7 KB) once per block
+  {
+    const double* src = reinterpret_cast<const double*>(P.tabs);
+    double* dst = reinterpret_cast<double*>(&tabs);
+    for (int i = threadIdx.x; i < (int)(sizeof(MathTabs) / sizeof(double)); i += kThreads) dst[i] = src[i];
+  }
+
+  int b = blockIdx.x;
+  const int chunk = b % P.ksplit;  b /= P.ksplit;
+  const int td = b % P.ntile_d;    b /= P.ntile_d;
+  const int th = b % P.ntile_h;
+  const int iq = b / P.ntile_h;
+  const int cg = chunk % P.ncg, rs = chunk / P.ncg;
+
+  const int bx = 1 << P.bx_log2;
+  const int col = cg * bx + (threadIdx.x & (bx - 1));
+  const int rsub = threadIdx.x >> P.bx_log2;
+  const int by = kThreads >> P.bx_log2;
+  const bool valid = col < P.N;
+
+  double hv[TH], d2v[TD];
+#pragma unroll
+  for (int i = 0; i < TH; ++i) hv[i] = P.h[min(th * TH + i, P.nh - 1)];
+#pragma unroll
+  for (int j = 0; j < TD; ++j) d2v[j] = P.d2[min(td * TD + j, P.nd - 1)];
+
+  double acc[TH][TD];
+#pragma unroll
+  for (int i = 0; i < TH; ++i)
+#pragma unroll
+    for (int j = 0; j < TD; ++j) acc[i][j] = 0.0;
+
+  __syncthreads();   // tables staged
+
+  const unsigned wmask = __ballot_sync(0xffffffffu, valid);
+  if (valid) {
+    const double4 ct = P.coltab[(size_t)iq * P.N + col];
+    const double4* rt = P.rowtab + (size_t)iq * P.N;
+    const int r0 = rs * P.rows_per_chunk;
+    const int r1 = min(P.N, r0 + P.rows_per_chunk);
+    const double T = P.T, nb = P.neg_beta;
+
+    for (int r = r0 + rsub; r < r1; r += by) {
+      const double4 rr = rt[r];
+      double Ek[NB], Eq[NB];
+      band_energies<NB>(P.mc, ct.x, ct.y, rr.x, rr.y, Ek);     // E(k)
+      band_energies<NB>(P.mc, ct.z, ct.w, rr.z, rr.w, Eq);     // E(k - q) = E(-k + q)
+      double g2 = P.mc.eta_scale;                              // eta(k)            (S4)
+      if (FORM == 1) g2 *= ct.x * rr.x;
+      g2 *= g2;
+
+      double sA[NB], dA[NB];
+#pragma unroll
+      for (int e = 0; e < NB; ++e) {
+        sA[e] = fma(0.5, Ek[e] + Eq[e], -P.mc.mu);             // (a + b)/2          (S3)
+        dA[e] = 0.5 * (Ek[e] - Eq[e]);                         // (a - b)/2 + h
+      }
+#pragma unroll 1
+      for (int e = 0; e < NB; ++e) {
+        if (!((P.mc.band_mask >> e) & 1)) continue;
+        const double s = (e == 0) ? sA[0] : sA[NB - 1];        // selects, not local-memory indexing
+        const double d0 = (e == 0) ? dA[0] : dA[NB - 1];
+        const double s2 = s * s;
+        double R[TD];
+#pragma unroll
+        for (int j = 0; j < TD; ++j) R[j] = sqrt(fma(d2v[j], g2, s2));   // Eq. 4 radicand   (S5)
+#pragma unroll
+        for (int i = 0; i < TH; ++i) {
+          const double ad = fabs(d0 - hv[i]);                  // |d|
+          if (MODE == 1) {
+            bool in_window = false;
+#pragma unroll
+            for (int j = 0; j < TD; ++j) in_window |= (fabs(R[j] - ad) < P.window);
+            if (!__any_sync(wmask, in_window)) {
+#pragma unroll
+              for (int j = 0; j < TD; ++j) acc[i][j] += fmax(R[j], ad);
+              continue;
+            }
+          }
+#pragma unroll
+          for (int j = 0; j < TD; ++j) {
+            const double x1 = fabs(R[j] - ad);
+            const double x2 = R[j] + ad;
+            const double m = fmax(R[j], ad);
+            const double u = exp_nonpos(x1 * nb, tabs);
+            const double v = exp_nonpos(x2 * nb, tabs);
+            const double w = fma(u, v, u + v);
+            const double l = log_1p_w(w, tabs);
+            acc[i][j] += fma(T, l, m);                          // -(f(E+) + f(E-) + b - s)   (S6)
+          }
+        }
+      }
+    }
+  }
+
+  // S8: fixed shuffle tree per accumulator, then fixed-order sum over the 8 warps.
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int i = 0; i < TH; ++i)
+#pragma unroll
+    for (int j = 0; j < TD; ++j) {
+      const double v = warp_sum(acc[i][j]);
+      if (lane == 0) red[warp][i * TD + j] = v;
+    }
+  __syncthreads();
+  if (threadIdx.x < TH * TD) {
+    const int i = threadIdx.x / TD, j = threadIdx.x % TD;
+    const int ih = th * TH + i, id = td * TD + j;
+    if (ih < P.nh && id < P.nd) {
+      double tot = 0.0;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) tot += red[w][threadIdx.x];
+      const size_t nout = (size_t)P.nq * P.nh * P.nd;
+      P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = tot;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// K2: Omega[o] = (S[iq] - sum_c partial[c][o]) + condc * Delta^2, chunks and S-chunks summed in index order.
+// ---------------------------------------------------------------------------------------------------
+__global__ void fe_finish_kernel(int nq, int nh, int nd, int ksplit, int nschunk, double condc,
+                                 const double* __restrict__ partial, const double* __restrict__ spart,
+                                 const double* __restrict__ d2, double* __restrict__ omega) {
+  const size_t nout = (size_t)nq * nh * nd;
+  const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= nout) return;
+  const int id = (int)(o % nd);
+  const int iq = (int)(o / ((size_t)nh * nd));
+  double S = 0.0;
+  for (int c = 0; c < nschunk; ++c) S += spart[(size_t)iq * nschunk + c];
+  double Psum = 0.0;
+  for (int c = 0; c < ksplit; ++c) Psum += partial[(size_t)c * nout + o];
+  omega[o] = fma(condc, d2[id], S - Psum);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// K3: argmin over Delta, one warp per (q, h) column.  (value, index) lexicographic minimum; NaN never wins.
+// ---------------------------------------------------------------------------------------------------
+__global__ void fe_argmin_kernel(int ncol, int nd, const double* __restrict__ omega, const double* __restrict__ delta,
+                                 int32_t* __restrict__ idx_out, double* __restrict__ dstar, double* __restrict__ ostar) {
+  const int col = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (col >= ncol) return;
+  const int lane = threadIdx.x & 31;
+  const double* om = omega + (size_t)col * nd;
+  double best = __longlong_as_double(0x7ff0000000000000LL);   // +inf
+  int bi = 0x7fffffff;
+  for (int i = lane; i < nd; i += 32) {
+    const double v = om[i];
+    if (v < best) { best = v; bi = i; }        // strided scan is ascending in i per lane: first occurrence kept
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double ov = __shfl_down_sync(0xffffffffu, best, o);
+    const int oi = __shfl_down_sync(0xffffffffu, bi, o);
+    if (ov < best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+  }
+  if (lane == 0) {
+    if (bi == 0x7fffffff) { bi = 0; best = om[0]; }   // all NaN / +inf column: report index 0
+    if (idx_out) idx_out[col] = bi;
+    if (dstar) dstar[col] = delta[bi];
+    if (ostar) ostar[col] = best;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// FP64 peak probe: 16 independent DFMA chains per thread, register-resident.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fe_dfma_probe_kernel(int iters, double seed, double* __restrict__ sink) {
+  double a[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) a[i] = seed + (double)(threadIdx.x + i);
+  const double m = 1.0000000001, c = 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = fma(a[i], m, c);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += a[i];
+  if (s == 12345.678) sink[0] = s;    // never true; keeps the chains alive
+}
+
+// Diagnostic: evaluate the device math on arrays (tests/test_fe_gpu.py::test_device_math).
+__global__ void fe_math_probe_kernel(int which, int n, const double* __restrict__ x, double* __restrict__ y,
+                                     const MathTabs* __restrict__ gtabs) {
+  __shared__ MathTabs tabs;
+  {
+    const double* src = reinterpret_cast<const double*>(gtabs);
+    double* dst = reinterpret_cast<double*>(&tabs);
+    for (int i = threadIdx.x; i < (int)(sizeof(MathTabs) / sizeof(double)); i += blockDim.x) dst[i] = src[i];
+  }
+  __syncthreads();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  y[i] = which == 0 ? exp_nonpos(x[i], tabs) : log_1p_w(x[i], tabs);
+}
+
+}  // namespace fe

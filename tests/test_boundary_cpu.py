@@ -1,0 +1,96 @@
+"""CPU-only checks of the C-ABI boundary: libfe.so loads without a GPU and exports every symbol
+include/fe.h declares; struct layouts of the two independent parameter structs agree with the dict
+made by workloads.model_params.  No compute calls here (no GPU)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1412_8754_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "fe.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(fe_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_loads_without_gpu_and_exports_all_declared_symbols():
+    from paper_1412_8754_b200 import fe
+    L = fe.lib()
+    names = declared_functions()
+    assert "fe_create" in names and "fe_omega_grid" in names and "fe_argmin" in names
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/fe.h but not exported by libfe.so"
+    assert sorted(fe.EXPORTS) == names
+
+
+def test_no_python_level_fallback_in_binding():
+    """The binding must not import the oracle or numpy-compute the path."""
+    src = open(os.path.join(ROOT, "paper_1412_8754_b200", "fe.py")).read()
+    assert "oracle" not in src.replace("no CPU fallback", "")
+    for f in os.listdir(os.path.join(ROOT, "paper_1412_8754_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_1412_8754_b200", "csrc", f)).read().lower()
+
+
+def test_param_struct_matches_header_layout():
+    from paper_1412_8754_b200 import fe
+    s = fe.make_params(W.model_params(U=3.5, const_mode=1, band_mask=2, cond_mult=1.0))
+    assert C.sizeof(s) == 4 + 4 + 32 + 8 * 4 + 4 + 4      # 80 bytes, no hidden padding surprises
+    assert (s.model, s.form_factor, s.band_mask, s.const_mode) == (2, 1, 2, 1)
+    assert list(s.t) == list(W.TWO_BAND_T) and s.U == 3.5 and s.mu == W.TWO_BAND_MU
+
+
+def test_strerror_and_host_only_validation():
+    """Argument validation that happens before any CUDA call works without a GPU."""
+    from paper_1412_8754_b200 import fe
+    L = fe.lib()
+    assert L.fe_strerror(0) == b"ok"
+    out = C.c_void_p()
+    p = fe.make_params(W.model_params())
+    assert L.fe_create(None, 8, 0.1, C.byref(out)) == fe.FE_EINVAL
+    assert L.fe_create(C.byref(p), 0, 0.1, C.byref(out)) == fe.FE_EINVAL
+    assert L.fe_create(C.byref(p), 8, 0.0, C.byref(out)) == fe.FE_EINVAL          # T = 0 (reading G7)
+    assert L.fe_create(C.byref(p), 8, float("nan"), C.byref(out)) == fe.FE_EINVAL
+    bad = fe.make_params(W.model_params(U=0.0))
+    assert L.fe_create(C.byref(bad), 8, 0.1, C.byref(out)) == fe.FE_EINVAL
+    bad = fe.make_params(dict(W.model_params(), model=3))
+    assert L.fe_create(C.byref(bad), 8, 0.1, C.byref(out)) == fe.FE_EINVAL
+    assert b"model" in L.fe_strerror(fe.FE_EINVAL)
+    assert L.fe_set_temperature(None, 0.1) == fe.FE_EINVAL
+    assert L.fe_tile_info(0, None, None) == fe.FE_EINVAL
+    assert len(fe.tiles()) >= 2
+    L.fe_destroy(None)                                                              # no-op
+
+
+def test_create_fails_loudly_without_a_b200():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_1412_8754_b200 import fe
+    with pytest.raises(fe.FeError) as ei:
+        fe.FreeEnergy(W.model_params(), 16, 0.01)
+    assert ei.value.code in (fe.FE_ECUDA, fe.FE_EARCH)
+
+
+def test_workload_shapes_match_baseline_configs():
+    sizes = {1: (32, 1, 1, 64), 2: (128, 1, 16, 256), 3: (512, 64, 32, 256), 4: (1024, 32, 64, 512),
+             5: (4096, 16, 16, 1024)}
+    for i, (N, nq, nh, nd) in sizes.items():
+        w = W.config(i)
+        assert (w.N, w.nq, w.nh, w.nd) == (N, nq, nh, nd)
+    w4 = W.config(4)
+    assert w4.T == (0.001, 0.01) and np.allclose(w4.q[:, 0], w4.q[:, 1]) and abs(w4.q[-1, 0] - 0.2 * np.pi) < 1e-15
+    assert w4.k_param_evals() == 1024 * 1024 * 32 * 64 * 512
+    w5a, w5b = W.config(5, seed=1), W.config(5, seed=2)
+    ta, tb = np.array(w5a.params["t"]), np.array(w5b.params["t"])
+    assert np.all(np.abs(ta / np.array(W.TWO_BAND_T) - 1) <= 0.01) and not np.array_equal(ta, tb)
+    assert W.config(5, seed=1).params["t"] == w5a.params["t"]          # seeded: reproducible
+    cols = W.sample_columns(w4, 16, 4)
+    assert len(set(cols)) == 16 and (0, 0) in cols and (31, 63) in cols
+    pts = W.sample_points(w4, 40, 4)
+    assert len(set(pts)) == 40 and all(0 <= a < 32 and 0 <= b < 64 and 0 <= c < 512 for a, b, c in pts)
