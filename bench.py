@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Omega(Delta; q, h, T) hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mode dense|windowed]
+
+Workload (config.workload): BASELINE.json configs[3] "cfg4_fflo_N1024": two-band s+- model, N = 1024 x 1024 k-grid,
+32 q along (1,1), 64 h, 512 Delta -- the configuration north_star quotes its FP64-roofline target on.
+One STEP = one pass of the whole hot path over one batch: fe_omega_grid (K0 trig, KS constant sum, K1 k-sum,
+K2 finish) + fe_argmin over the batch's full (q, h, Delta) grid at one temperature; successive steps alternate
+T = 0.001 / 0.01 (config 4 names both).  The batch is `--q-per-step` q-values of the config (default: all 32),
+so a default step is the whole 1.1e12-evaluation scan.
+
+Output: ONE JSON line (rank 0).  value = k-point x parameter evaluations per second, whole job, inputs resident
+(device timing with CUDA events per step, L2 flushed between steps, max over ranks).  e2e = same metric through
+fe_scan_host with HOST buffers (lists H2D, Omega + minima D2H inside the timed region).
+roofline: bound "alu" (plain FP64 pipe; no contraction, HBM negligible), see DESIGN.md "Roofline".
+cpu_baseline: the oracle (oracle/fe_oracle.c) as it stands, timed on this host's cores on a bounded sample.
+`--impl reference` times the oracle instead (the reference arm of this tier).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1412_8754_b200 import workloads as W  # noqa: E402
+
+METRIC = "Omega evaluations/s (k-points x grid points, fp64)"
+UNIT = "k-point x (q,h,Delta) evaluations/s"
+
+# FP64-pipe instructions and flops per (k, band, q, h, Delta) term of the K1 kernel as built (
+# counted from cuobjdump -sass of the dense kernel's band-loop body, tile overheads included).
+KERNEL_COUNTS = {
+    # tile (TH, TD): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1, DSETP = 0]) per band-eval
+    (4, 4): (40.6, 61.3),
+    (8, 4): (39.4, 59.4),
+}
+SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
+PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
+PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
+
+
+# ----------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        hot = [s for s in sm if s > 0.5 * (max(mx) if mx else 1)] or sm
+        return {"sm_mhz": statistics.median(hot) if hot else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(w, T, n_delta, nthreads=None):
+    """Time the oracle on ONE (q, h) column of the workload with the first n_delta... evenly spaced Delta values."""
+    from oracle import fe_oracle as O
+    if nthreads:
+        O.set_num_threads(nthreads)
+    ids = np.unique(np.linspace(0, w.nd - 1, n_delta).round().astype(int))
+    iq, ih = w.nq // 2, w.nh // 2
+    t0 = time.perf_counter()
+    O.omega_column(w.params, w.N, T, w.q[iq], w.h[ih], w.delta[ids])
+    dt = time.perf_counter() - t0
+    evals = w.N * w.N * len(ids)
+    return evals / dt, dt, len(ids), O.num_threads(), (iq, ih)
+
+
+def run_reference(args, w):
+    """Reference arm of this tier: the oracle on the host cores, same metric/config; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    T = w.T[0]
+    n_delta = args.ref_deltas
+    for _ in range(args.warmup):
+        oracle_sample(w, T, max(2, n_delta // 8))
+    times, evals = [], 0
+    for _ in range(args.steps):
+        v, dt, nd_used, cores, col = oracle_sample(w, T, n_delta)
+        times.append(dt)
+        evals += w.N * w.N * nd_used
+    value = evals / sum(times)
+    sample = (f"per step: 1 of {w.nq * w.nh} (q,h) columns (iq={col[0]}, ih={col[1]}) x {nd_used} of {w.nd} Delta, "
+              f"full {w.N}x{w.N} k-sum, T={T}")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "nq": w.nq, "nh": w.nh, "nd": w.nd, "T": list(w.T)},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mode", default="dense", choices=["dense", "windowed"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--q-per-step", type=int, default=0, help="q-values per step (0 = the whole q list)")
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--ref-deltas", type=int, default=64)
+    ap.add_argument("--cpu-baseline-deltas", type=int, default=256)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    w = W.config(args.config)
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1412_8754_b200 import fe
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: no CUDA device visible (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    fe.lib()
+
+    # ---- workload of this rank (weak scaling: every rank scans nq q-values of a `world`-times finer q grid) ----
+    nq_step = args.q_per_step or w.nq
+    if world > 1:
+        qfine = np.linspace(w.q[0], w.q[-1], w.nq * world)
+        q_all = qfine[rank::world]
+    else:
+        q_all = w.q
+    temps = list(w.T)
+    mode = fe.EVAL_DENSE if args.mode == "dense" else fe.EVAL_WINDOWED
+
+    F = fe.FreeEnergy(w.params, w.N, temps[0])
+    F.set_eval_mode(mode)
+    F.set_tuning(args.tile, 0)
+    F.enable_timing(True)
+    stream = torch.cuda.current_stream()
+    omega = torch.empty((nq_step, w.nh, w.nd), dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")    # 256 MB > 126 MB L2
+
+    def q_of(step):
+        s = (step * nq_step) % len(q_all)
+        return np.ascontiguousarray(np.take(q_all, range(s, s + nq_step), axis=0, mode="wrap"))
+
+    def one_step(step):
+        F.set_temperature(temps[step % len(temps)])
+        F.omega_grid(q_of(step), w.h, w.delta, out=omega, stream=stream)
+        return F.argmin(omega, w.delta, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    evals_per_step = w.N * w.N * nq_step * w.nh * w.nd
+    for s in range(args.warmup):
+        one_step(s)
+    barrier()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = F.launch_count()
+    step_ms, ksum_ms, band_evals = [], [], 0.0
+    barrier()
+    t_wall0 = time.perf_counter()
+    for s in range(args.steps):
+        flush.zero_()                                   # L2 flush between timed iterations (outside the events)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        res = one_step(args.warmup + s)
+        e1.record(stream)
+        e1.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        ms, be = F.last_ksum()
+        ksum_ms.append(ms)
+        band_evals = be
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = F.launch_count() - launches0
+    clocks = sampler.stop()
+    idx_check = int(res[0].sum().item())               # device->host read of the step's result
+
+    total_ms = sum(step_ms)
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    value = evals_per_step * args.steps * world / (total_ms_max * 1e-3)
+
+    # ---- e2e: host buffers through fe_scan_host (pinned), copies inside the timed region ----
+    pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()    # noqa: E731
+    out = dict(omega=pin((nq_step, w.nh, w.nd), torch.float64), idx=pin((nq_step, w.nh), torch.int32),
+               delta_star=pin((nq_step, w.nh), torch.float64), omega_star=pin((nq_step, w.nh), torch.float64))
+    hq = [pin((nq_step, 2), torch.float64) for _ in range(2)]
+    hh, hd = pin((w.nh,), torch.float64), pin((w.nd,), torch.float64)
+    hh[:] = w.h
+    hd[:] = w.delta
+    e2e_steps = max(1, min(args.steps, 2))
+    F.set_temperature(temps[0])
+    hq[0][:] = q_of(0)
+    F.scan_host(hq[0], hh, hd, out=out, stream=stream)              # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(e2e_steps):
+        F.set_temperature(temps[s % len(temps)])
+        hq[s % 2][:] = q_of(s)
+        F.scan_host(hq[s % 2], hh, hd, out=out, stream=stream)      # synchronous: returns with results on the host
+    torch.cuda.synchronize()
+    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = evals_per_step * e2e_steps * world / float(te.item())
+    h2d = 8 * (2 * nq_step + w.nh + 2 * w.nd)           # q, h, Delta^2 lists + Delta list for the argmin
+    d2h = 8 * nq_step * w.nh * w.nd + nq_step * w.nh * (4 + 8 + 8)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (K1 k-sum) ----
+    th_td = fe.tiles()[args.tile - 1] if args.tile else fe.tiles()[0] if w.nh % 8 == 0 else None
+    counts = KERNEL_COUNTS.get(tuple(th_td) if th_td else None, (None, None))
+    k_ms = sum(ksum_ms) / len(ksum_ms)
+    dfma_rate, _ = fe.fp64_peak_probe()
+    roofline = {"bound": "alu", "kernel": "fe_ksum_kernel (K1)", "unit": "TFLOP/s", "peak": PEAK_TFLOPS,
+                "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
+                "peak_measured_dfma_probe": 2 * dfma_rate / 1e12, "avg_launch_ms": k_ms,
+                "band_evals_per_launch": band_evals, "traffic": None,
+                "kernel_share_of_step": k_ms * len(ksum_ms) / total_ms}
+    if counts[0]:
+        achieved = band_evals * counts[1] / (k_ms * 1e-3) / 1e12
+        roofline.update({"achieved": achieved, "frac": achieved / PEAK_TFLOPS,
+                         "flop_per_band_eval": counts[1], "fp64_inst_per_band_eval": counts[0],
+                         "fp64_pipe_frac": band_evals * counts[0] / (k_ms * 1e-3) / PEAK_DFMA_PER_S,
+                         "frac_of_measured_dfma_peak": achieved / (2 * dfma_rate / 1e12)})
+    else:
+        roofline.update({"achieved": None, "frac": None})
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, dt, nd_used, cores, col = oracle_sample(w, temps[0], args.cpu_baseline_deltas)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": (f"1 of {w.nq * w.nh} (q,h) columns of {w.name} (iq={col[0]}, ih={col[1]}) x {nd_used} of "
+                          f"{w.nd} Delta, full {w.N}x{w.N} k-sum, T={temps[0]}")}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "model": None, "N": w.N, "nq_per_step": nq_step, "nh": w.nh, "nd": w.nd,
+                       "T_alternating": temps, "eval_mode": args.mode, "band_evals_per_step": evals_per_step * w.nbands,
+                       "l2": "flushed between timed steps (256 MB memset); inputs are a few KB",
+                       "parallelism": f"q-sharded x{world}, no collective on the data path"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps, "api": "fe_scan_host (host buffers in/out, synchronous)"},
+            "gpu_launches": launches, "wall_s_timed_region": t_wall, "clocks": clocks,
+            "roofline": roofline, "cpu_baseline": cpu, "result_check": idx_check}
+    del line["config"]["model"]
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
