@@ -144,7 +144,7 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="dense", choices=["dense", "windowed"])
+    ap.add_argument("--mode", default="factored", choices=["factored", "direct", "windowed"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--q-per-step", type=int, default=0, help="q-values per step (0 = the whole q list)")
     ap.add_argument("--tile", type=int, default=0)
@@ -179,7 +179,7 @@ def main():
     else:
         q_all = w.q
     temps = list(w.T)
-    mode = fe.EVAL_DENSE if args.mode == "dense" else fe.EVAL_WINDOWED
+    mode = {"factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT, "windowed": fe.EVAL_WINDOWED}[args.mode]
 
     F = fe.FreeEnergy(w.params, w.N, temps[0])
     F.set_eval_mode(mode)

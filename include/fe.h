@@ -46,13 +46,17 @@ extern "C" {
 #define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
 #define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
 
-/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode) ----
- * DENSE   : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5.
- * WINDOWED: a term whose thermal part is below half an ulp of its T=0 part (|R-|d|| >= 37 T)
- *           adds only max(R,|d|); the decision is taken per warp.  Same sums to rounding (bit-identical
- *           per term; only whole warps skip work).                                                        */
-#define FE_EVAL_DENSE    0
-#define FE_EVAL_WINDOWED 1
+/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all three compute the same sums ----
+ * FACTORED: default.  Uses 2cosh(d/T) + 2cosh(R/T) = B(h) + A(Delta): per (k, band) TH + TD exponentials in
+ *           extended range (fp64 mantissa + int exponent), per term one add and one multiply into a running
+ *           product; the logarithm is taken once per thread at the end.
+ * DIRECT  : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5
+ *           (the stable form max(R,|d|) + T ln(1 + u + v + uv)).
+ * WINDOWED: DIRECT, but a term whose thermal part is below half an ulp of its T=0 part (|R-|d|| >= 37 T) adds
+ *           only max(R,|d|); the decision is taken per warp.  Bit-identical to DIRECT.                      */
+#define FE_EVAL_FACTORED 0
+#define FE_EVAL_DIRECT   1
+#define FE_EVAL_WINDOWED 2
 
 typedef struct fe_handle fe_handle; /* opaque; owns device scratch (trig tables, partial sums, staging) */
 
@@ -77,7 +81,7 @@ int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** ou
 /* Change T (> 0, finite) for subsequent calls (config 4 scans two temperatures).  Host-only, cheap. */
 int fe_set_temperature(fe_handle* h, double T);
 
-/* Select FE_EVAL_DENSE (default) or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
+/* Select FE_EVAL_FACTORED (default), FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
 int fe_set_eval_mode(fe_handle* h, int32_t mode);
 
 /* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,

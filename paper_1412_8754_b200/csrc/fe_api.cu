@@ -46,7 +46,7 @@ struct fe_handle {
   fe_model_params p;
   int32_t N = 0;
   double T = 0;
-  int32_t mode = FE_EVAL_DENSE;
+  int32_t mode = FE_EVAL_FACTORED;
   int32_t tile = 0;            // 0 = auto, else 1 + index
   int32_t target_blocks = 0;   // 0 = auto
   int device = 0;
@@ -104,6 +104,7 @@ int validate_params(const fe_model_params* p, int32_t N, double T) {
 
 void build_tabs(MathTabs* t) {
   for (int j = 0; j < kExpTabN; ++j) t->exp2_j64[j] = (double)exp2l((long double)j / 64.0L);
+  for (int j = 0; j < 256; ++j) t->exp2_j256[j] = (double)exp2l((long double)j / 256.0L);
   for (int idx = 0; idx < kLogTabN; ++idx) {
     const int e = idx >> 7, i = idx & 127;
     const long double c = ldexpl(1.0L + ((long double)i + 0.5L) / 128.0L, e);
@@ -125,6 +126,21 @@ ModelConsts make_consts(const fe_model_params& p) {
   }
   mc.mu = p.mu; mc.eta_scale = p.eta_scale; mc.band_mask = p.band_mask; mc.const_mode = p.const_mode;
   return mc;
+}
+
+FactoredConsts make_factored(double T) {
+  FactoredConsts fc;
+  const long double ln2 = 0.693147180559945309417232121458176568L;
+  const long double c2 = (long double)T * ln2 / 256.0L;
+  fc.c1 = (double)(256.0L / ((long double)T * ln2));
+  fc.c2hi = (double)c2;
+  fc.c2lo = (double)(c2 - (long double)fc.c2hi);
+  const long double beta = 1.0L / (long double)T;
+  fc.b1 = (double)beta;
+  fc.b2 = (double)(beta * beta / 2.0L);
+  fc.b3 = (double)(beta * beta * beta / 6.0L);
+  fc.b4 = (double)(beta * beta * beta * beta / 24.0L);
+  return fc;
 }
 
 template <typename T>
@@ -188,8 +204,9 @@ int choose_tile(const fe_handle* h, int nh, int nd) {
 
 template <int NB, int FORM, int TH, int TD>
 cudaError_t launch_ksum_mode(int mode, int grid, cudaStream_t st, const KsumParams& P) {
-  if (mode == FE_EVAL_WINDOWED) fe_ksum_kernel<NB, FORM, TH, TD, 1><<<grid, kThreads, 0, st>>>(P);
-  else                          fe_ksum_kernel<NB, FORM, TH, TD, 0><<<grid, kThreads, 0, st>>>(P);
+  if (mode == FE_EVAL_WINDOWED)    fe_ksum_kernel<NB, FORM, TH, TD, 1><<<grid, kThreads, 0, st>>>(P);
+  else if (mode == FE_EVAL_DIRECT) fe_ksum_kernel<NB, FORM, TH, TD, 0><<<grid, kThreads, 0, st>>>(P);
+  else                             fe_ksum_factored_kernel<NB, FORM, TH, TD><<<grid, kThreads, 0, st>>>(P, make_factored(P.T));
   return cudaGetLastError();
 }
 
@@ -260,6 +277,26 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   if (nrs < 1) nrs = 1;
   int rpc = (int)((N + nrs - 1) / nrs);
   rpc = (rpc + by - 1) / by * by;                // whole row-lane strides per chunk
+  {
+    // Range guards of the factored kernel: binary exponents x/(T ln2) are summed in int32 per thread, and the
+    // range reduction needs x/T * 64/ln2 < 2^37.  |E_k| <= W, so R <= W + |mu| + |Delta eta|, |d| <= W + |h|.
+    const fe_model_params& mp = h->p;
+    const double Wb = mp.model == FE_MODEL_ONE_BAND ? 4.0 * fabs(mp.t[0])
+                    : 2.0 * (fabs(mp.t[0]) + fabs(mp.t[1])) + 4.0 * fabs(mp.t[2]) + 4.0 * fabs(mp.t[3]);
+    double hmax = 0, dmax = 0;
+    for (int i = 0; i < nh; ++i) hmax = fmax(hmax, fabs(h_list[i]));
+    for (int i = 0; i < nd; ++i) dmax = fmax(dmax, fabs(delta[i]));
+    const double xmax = fmax(Wb + fabs(mp.mu) + dmax * fabs(mp.eta_scale), Wb + hmax) / h->T;
+    if (!(xmax < 1.0e9)) {
+      snprintf(g_errbuf, sizeof g_errbuf, "T = %g is too small for the energy scale (max x/T = %.3g >= 1e9)", h->T, xmax);
+      return FE_EINVAL;
+    }
+    const double ebound = xmax / 0.6931471805599453 + 4.0;            // max binary exponent of one term
+    const double max_terms = 2.0e9 / ebound;                          // per thread and accumulator
+    int max_rows = (int)fmin((double)N, floor(max_terms / h->nb)) * by;
+    if (max_rows < by) max_rows = by;
+    if (rpc > max_rows) rpc = max_rows / by * by;
+  }
   P.rows_per_chunk = rpc;
   P.nrs = (N + rpc - 1) / rpc;
   P.ksplit = P.ncg * P.nrs;
@@ -373,7 +410,7 @@ int fe_set_temperature(fe_handle* h, double T) {
 
 int fe_set_eval_mode(fe_handle* h, int32_t mode) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
-  if (mode != FE_EVAL_DENSE && mode != FE_EVAL_WINDOWED) {
+  if (mode != FE_EVAL_FACTORED && mode != FE_EVAL_DIRECT && mode != FE_EVAL_WINDOWED) {
     snprintf(g_errbuf, sizeof g_errbuf, "unknown eval mode %d", mode); return FE_EINVAL; }
   h->mode = mode;
   return FE_OK;

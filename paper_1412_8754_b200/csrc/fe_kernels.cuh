@@ -266,6 +266,228 @@ __global__ void __launch_bounds__(kThreads) fe_ksum_kernel(const KsumParams P) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// K1f: the k-sum in FACTORED form (default).  Same quantity as K1, P = sum_k T ln Z, Z = 2cosh(d/T) + 2cosh(R/T),
+// but uses that Z is a SUM of a Delta-only and an h-only term:
+//     Z_ij = A_j + B_i,   A_j = 2cosh(R_j/T) = mA_j 2^{eA_j},   B_i = 2cosh(|d_i|/T) = mB_i 2^{eB_i}
+// (extended-range numbers: fp64 mantissa in [0.99, 2.6) and an int32 binary exponent, so R/T ~ 10^4 is no problem).
+// Per (k, band) a thread evaluates TD + TH exponentials instead of 2 TH TD, and NO logarithm: it keeps a running
+// PRODUCT accP_ij of the (rescaled) Z_ij and integer sums of the binary exponents taken out, and takes one
+// logarithm per accumulator at the very end:  P_ij = T (ln2 * exponent_sum_ij + ln accP_ij).
+//   fast path  (whole warp: every pair's exponent within kSpread of the tile maximum Eref):
+//        A'_j = A_j 2^-Eref, B'_i = B_i 2^-Eref once per (k, band);  per pair: accP_ij *= (A'_j + B'_i)   [DADD + DMUL]
+//        one shared integer accumulator  accEc += Eref.
+//   robust path (any lane fails the test, e.g. |d| dominates and the h-tile spans many binades):
+//        per pair E = max(eA_j, eB_i), both mantissas shifted to E, accP_ij *= sum, accE_ij += E with accE in
+//        shared memory ([pair][thread], conflict-free).
+// accP is renormalised every kRenorm rows (its exponent moved into accEc ... see code).  (DESIGN.md "K1f".)
+// ---------------------------------------------------------------------------------------------------
+constexpr int kRenorm = 32;   // rows between renormalisations: <= 64 factors in [2^-9, 5.2): 2^-576 .. 2^153
+constexpr int kSpread = 8;    // fast path: all pair exponents within 2^-8 of the tile maximum
+
+struct FactoredConsts {       // per-temperature constants of the extended-range exponential (host, long double)
+  double c1;                  // 256 / (T ln2):        n = rint(x c1)
+  double c2hi, c2lo;          // T ln2 / 256 (split):  r = x - n c2   (energy units, |r| <= T ln2 / 512)
+  double b1, b2, b3, b4;      // beta^k / k!:          e^{r/T} - 1 = r (b1 + r (b2 + r (b3 + r b4)))
+};
+
+// Mantissa of e^{x/T} 2^{-(n>>8)} in [0.997, 2) given t = fma(x, c1, MAGIC).
+__device__ __forceinline__ double exp_mant(double x, double t, const FactoredConsts& fc, const double* __restrict__ tab256) {
+  const double MAGIC = 6755399441055744.0;        // 1.5 * 2^52
+  const double nf = t - MAGIC;
+  double r = fma(nf, -fc.c2hi, x);
+  r = fma(nf, -fc.c2lo, r);
+  double p = fma(r, fc.b4, fc.b3);
+  p = fma(p, r, fc.b2);
+  p = fma(p, r, fc.b1);
+  p = p * r;                                      // e^{r/T} - 1, truncation (r/T)^5/120 < 3.8e-17
+  const double s = tab256[__double2loint(t) & 255];
+  return fma(s, p, s);
+}
+
+// e^{x/T} + e^{-x/T} = 2^k (m + 2^{-2k}/m): add the second term to the mantissa (only matters for k < 28).
+__device__ __forceinline__ double cosh_fix(double m, int k) {
+  double rc;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(m));
+  double e = fma(-m, rc, 1.0);
+  rc = fma(rc, e, rc);
+  e = fma(-m, rc, 1.0);
+  rc = fma(rc, e, rc);                            // 1/m to ~1 ulp
+  const int kk = min(k, 400);
+  const double sc = __hiloint2double((1023 - 2 * kk) << 20, 0);
+  return fma(rc, sc, m);                          // in [0.997, 2.51)
+}
+
+__device__ __forceinline__ int exp_k(double t) {  // n >> 8 from the 52-bit mantissa of t = MAGIC + n (0 <= n < 2^39)
+  return __funnelshift_r(__double2loint(t), __double2hiint(t), 8);
+}
+
+__device__ __forceinline__ double scale2(double m, int shift) {   // m * 2^shift, shift <= 0, flushed at 2^-1000
+  const int s = max(shift, -1000);
+  return __hiloint2double(__double2hiint(m) + (s << 20), __double2loint(m));
+}
+
+template <int NB, int FORM, int TH, int TD>
+__global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
+  __shared__ double tab256[256];
+  __shared__ double hv_s[TH], d2v_s[TD];
+  __shared__ int accE_s[TH * TD][kThreads];        // robust-path exponent sums, [pair][thread]
+  __shared__ double red[kWarps][TH * TD];
+  for (int i = threadIdx.x; i < 256; i += kThreads) tab256[i] = P.tabs->exp2_j256[i];
+#pragma unroll
+  for (int pq = 0; pq < TH * TD; ++pq) accE_s[pq][threadIdx.x] = 0;
+
+  int b = blockIdx.x;
+  const int chunk = b % P.ksplit;  b /= P.ksplit;
+  const int td = b % P.ntile_d;    b /= P.ntile_d;
+  const int th = b % P.ntile_h;
+  const int iq = b / P.ntile_h;
+  const int cg = chunk % P.ncg, rs = chunk / P.ncg;
+
+  const int bx = 1 << P.bx_log2;
+  const int col = cg * bx + (threadIdx.x & (bx - 1));
+  const int rsub = threadIdx.x >> P.bx_log2;
+  const int by = kThreads >> P.bx_log2;
+  const bool valid = col < P.N;
+
+  if (threadIdx.x < TH) hv_s[threadIdx.x] = P.h[min(th * TH + (int)threadIdx.x, P.nh - 1)];
+  if (threadIdx.x < TD) d2v_s[threadIdx.x] = P.d2[min(td * TD + (int)threadIdx.x, P.nd - 1)];
+
+  double accP[TH][TD];
+#pragma unroll
+  for (int i = 0; i < TH; ++i)
+#pragma unroll
+    for (int j = 0; j < TD; ++j) accP[i][j] = 1.0;
+  int accEc = 0;                                   // exponent sum common to all pairs of this thread
+
+  __syncthreads();
+
+  const double MAGIC = 6755399441055744.0;
+  const unsigned wmask = __ballot_sync(0xffffffffu, valid);
+  if (valid) {
+    const double4 ct = P.coltab[(size_t)iq * P.N + col];
+    const double4* rt = P.rowtab + (size_t)iq * P.N;
+    const int r0 = rs * P.rows_per_chunk;
+    const int r1 = min(P.N, r0 + P.rows_per_chunk);
+
+    for (int rb = r0 + rsub; rb < r1; rb += by * kRenorm) {
+      const int rend = min(r1, rb + by * kRenorm);
+      for (int r = rb; r < rend; r += by) {
+        const double4 rr = rt[r];
+        double Ek[NB], Eq[NB];
+        band_energies<NB>(P.mc, ct.x, ct.y, rr.x, rr.y, Ek);
+        band_energies<NB>(P.mc, ct.z, ct.w, rr.z, rr.w, Eq);
+        double g2 = P.mc.eta_scale;
+        if (FORM == 1) g2 *= ct.x * rr.x;
+        g2 *= g2;
+        double sA[NB], dA[NB];
+#pragma unroll
+        for (int e = 0; e < NB; ++e) {
+          sA[e] = fma(0.5, Ek[e] + Eq[e], -P.mc.mu);
+          dA[e] = 0.5 * (Ek[e] - Eq[e]);
+        }
+#pragma unroll 1
+        for (int e = 0; e < NB; ++e) {
+          if (!((P.mc.band_mask >> e) & 1)) continue;
+          const double s = (e == 0) ? sA[0] : sA[NB - 1];
+          const double d0 = (e == 0) ? dA[0] : dA[NB - 1];
+          const double s2 = s * s;
+
+          // ---- pass 1: binary exponents of all A_j, B_i ----
+          double mA[TD];
+          int eA[TD], eB[TH];
+          int emaxA = 0, eminA = 0x7fffffff, emaxB = 0, eminB = 0x7fffffff;
+#pragma unroll
+          for (int j = 0; j < TD; ++j) {
+            const double R = sqrt(fma(d2v_s[j], g2, s2));                  // Eq. 4 radicand
+            const double t = fma(R, fc.c1, MAGIC);
+            eA[j] = exp_k(t);
+            mA[j] = exp_mant(R, t, fc, tab256);
+            emaxA = max(emaxA, eA[j]); eminA = min(eminA, eA[j]);
+          }
+          if (__any_sync(wmask, eminA < 28)) {
+#pragma unroll
+            for (int j = 0; j < TD; ++j) mA[j] = cosh_fix(mA[j], eA[j]);
+          }
+#pragma unroll
+          for (int i = 0; i < TH; ++i) {
+            const double t = fma(fabs(d0 - hv_s[i]), fc.c1, MAGIC);
+            eB[i] = exp_k(t);
+            emaxB = max(emaxB, eB[i]); eminB = min(eminB, eB[i]);
+          }
+          const int Eref = max(emaxA, emaxB);
+          const bool fixB = __any_sync(wmask, eminB < 28);
+          const bool fast = __all_sync(wmask, max(eminA, eminB) >= Eref - kSpread);
+
+          if (fast) {
+            accEc += Eref;
+            double Ap[TD];
+#pragma unroll
+            for (int j = 0; j < TD; ++j) Ap[j] = scale2(mA[j], eA[j] - Eref);
+#pragma unroll
+            for (int i = 0; i < TH; ++i) {
+              const double ad = fabs(d0 - hv_s[i]);
+              double mB = exp_mant(ad, fma(ad, fc.c1, MAGIC), fc, tab256);
+              if (fixB) mB = cosh_fix(mB, eB[i]);
+              const double Bp = scale2(mB, eB[i] - Eref);
+#pragma unroll
+              for (int j = 0; j < TD; ++j) accP[i][j] *= (Ap[j] + Bp);
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < TH; ++i) {
+              const double ad = fabs(d0 - hv_s[i]);
+              double mB = exp_mant(ad, fma(ad, fc.c1, MAGIC), fc, tab256);
+              if (fixB) mB = cosh_fix(mB, eB[i]);
+#pragma unroll
+              for (int j = 0; j < TD; ++j) {
+                const int E = max(eA[j], eB[i]);
+                accP[i][j] *= (scale2(mA[j], eA[j] - E) + scale2(mB, eB[i] - E));
+                accE_s[i * TD + j][threadIdx.x] += E;
+              }
+            }
+          }
+        }
+      }
+      // renormalise: move the binary exponent of each running product into the integer sums
+#pragma unroll
+      for (int i = 0; i < TH; ++i)
+#pragma unroll
+        for (int j = 0; j < TD; ++j) {
+          const int hi = __double2hiint(accP[i][j]);
+          const int ex = (hi >> 20) - 1023;
+          accE_s[i * TD + j][threadIdx.x] += ex;
+          accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
+        }
+    }
+  }
+
+  // per-thread P = T (ln2 * exponent sum + ln accP), then the same fixed-order reduction as K1
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const double LN2_HI = 6.93147180369123816490e-01, LN2_LO = 1.90821492927058770002e-10;
+#pragma unroll
+  for (int i = 0; i < TH; ++i)
+#pragma unroll
+    for (int j = 0; j < TD; ++j) {
+      const double ed = (double)accEc + (double)accE_s[i * TD + j][threadIdx.x];
+      const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(accP[i][j])));
+      const double v = warp_sum(P.T * lnz);
+      if (lane == 0) red[warp][i * TD + j] = v;
+    }
+  __syncthreads();
+  if (threadIdx.x < TH * TD) {
+    const int i = threadIdx.x / TD, j = threadIdx.x % TD;
+    const int ih = th * TH + i, id = td * TD + j;
+    if (ih < P.nh && id < P.nd) {
+      double tot = 0.0;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) tot += red[w][threadIdx.x];
+      const size_t nout = (size_t)P.nq * P.nh * P.nd;
+      P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = tot;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // K2: Omega[o] = (S[iq] - sum_c partial[c][o]) + condc * Delta^2, chunks and S-chunks summed in index order.
 // ---------------------------------------------------------------------------------------------------
 __global__ void fe_finish_kernel(int nq, int nh, int nd, int ksplit, int nschunk, double condc,

@@ -21,8 +21,9 @@ namespace fe {
 constexpr int kExpTabN = 64;    // 2^(j/64), j = 0..63
 constexpr int kLogTabN = 260;   // index = exponent and top 7 mantissa bits of y in [1, 4]: 0..256 reachable, padded
 
-struct MathTabs {               // lives in shared memory inside kernels; filled from global at kernel start
+struct MathTabs {               // global copy; kernels stage the parts they use in shared memory
   double  exp2_j64[kExpTabN];
+  double  exp2_j256[256];       // 2^(j/256), j = 0..255 (factored kernel)
   double2 log_tab[kLogTabN];    // .x = 2^-e / c,  .y = -ln(.x) rounded   (c = centre of the 1/128-wide mantissa bin)
 };
 

@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
-EVAL_DENSE, EVAL_WINDOWED = 0, 1
+EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED = 0, 1, 2
 
 EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_scan_host",
            "fe_enable_timing", "fe_get_timing", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info",
