@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Omega(Delta; q, h, T) hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mode dense|windowed]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mode factored|direct|windowed]
 
 Workload (config.workload): BASELINE.json configs[3] "cfg4_fflo_N1024": two-band s+- model, N = 1024 x 1024 k-grid,
 32 q along (1,1), 64 h, 512 Delta -- the configuration north_star quotes its FP64-roofline target on.
@@ -38,12 +38,14 @@ from paper_1412_8754_b200 import workloads as W  # noqa: E402
 METRIC = "Omega evaluations/s (k-points x grid points, fp64)"
 UNIT = "k-point x (q,h,Delta) evaluations/s"
 
-# FP64-pipe instructions and flops per (k, band, q, h, Delta) term of the K1 kernel as built (
-# counted from cuobjdump -sass of the dense kernel's band-loop body, tile overheads included).
+# FP64-pipe instructions and flops EXECUTED per (k, band, q, h, Delta) term by the k-sum kernel as built
+# (DESIGN.md "Roofline").  factored: ncu counters smsp__sass_thread_inst_executed_op_{dfma,dadd,dmul}_pred_on of the
+# cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
-    # tile (TH, TD): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1, DSETP = 0]) per band-eval
-    (4, 4): (40.6, 61.3),
-    (8, 4): (39.4, 59.4),
+    # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
+    ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
+    ("direct", (4, 4)): (40.6, 61.3, "SASS count"),
+    ("direct", (8, 4)): (39.4, 59.4, "SASS count"),
 }
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
@@ -270,11 +272,12 @@ def main():
         return
 
     # ---- roofline of the dominant kernel (K1 k-sum) ----
-    th_td = fe.tiles()[args.tile - 1] if args.tile else fe.tiles()[0] if w.nh % 8 == 0 else None
-    counts = KERNEL_COUNTS.get(tuple(th_td) if th_td else None, (None, None))
+    info = F.last_launch_info()
+    counts = KERNEL_COUNTS.get((args.mode, (info["th"], info["td"])), (None, None, None))
     k_ms = sum(ksum_ms) / len(ksum_ms)
     dfma_rate, _ = fe.fp64_peak_probe()
-    roofline = {"bound": "alu", "kernel": "fe_ksum_kernel (K1)", "unit": "TFLOP/s", "peak": PEAK_TFLOPS,
+    roofline = {"bound": "alu", "kernel": f"k-sum kernel ({args.mode}, tile {info['th']}x{info['td']}, grid {info['grid']} x 256)",
+                "unit": "TFLOP/s", "peak": PEAK_TFLOPS,
                 "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
                 "peak_measured_dfma_probe": 2 * dfma_rate / 1e12, "avg_launch_ms": k_ms,
                 "band_evals_per_launch": band_evals, "traffic": None,
@@ -282,7 +285,7 @@ def main():
     if counts[0]:
         achieved = band_evals * counts[1] / (k_ms * 1e-3) / 1e12
         roofline.update({"achieved": achieved, "frac": achieved / PEAK_TFLOPS,
-                         "flop_per_band_eval": counts[1], "fp64_inst_per_band_eval": counts[0],
+                         "flop_per_band_eval": counts[1], "fp64_inst_per_band_eval": counts[0], "counts_source": counts[2],
                          "fp64_pipe_frac": band_evals * counts[0] / (k_ms * 1e-3) / PEAK_DFMA_PER_S,
                          "frac_of_measured_dfma_peak": achieved / (2 * dfma_rate / 1e12)})
     else:

@@ -123,6 +123,10 @@ int fe_scan_host(fe_handle* h,
 int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
 
+/* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode,
+ * rows per k-chunk}.  Host-only. */
+int fe_get_last_launch_info(fe_handle* h, int32_t* info6);
+
 /* Number of kernel launches this handle has issued since creation (all kernels of this library). */
 int fe_get_launch_count(fe_handle* h, int64_t* launches);
 

@@ -72,6 +72,7 @@ struct fe_handle {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timing_valid = false;
   double last_band_evals = 0;
+  int32_t last_info[6] = {0, 0, 0, 0, 0, 0};   // th, td, ksplit, grid, mode, rows_per_chunk
   int64_t launches = 0;
 };
 
@@ -188,15 +189,19 @@ int stage_lists(fe_handle* h, size_t n, cudaStream_t st, double** host_out, doub
   return FE_OK;
 }
 
+// Relative cost per evaluated term of each tile (measured on B200, config-4 slice).
+// kTiles order: (8,4) (4,4) (2,8) (1,8).
+constexpr double kTileCostFactored[] = {1.00, 1.33, 1.76, 2.60};
+constexpr double kTileCostDirect[]   = {1.51, 1.00, 1.12, 1.30};
+
 int choose_tile(const fe_handle* h, int nh, int nd) {
   if (h->tile > 0) return h->tile - 1;
-  // least padded work; ties go to the earlier (larger / better amortised) tile
+  const double* cost_tab = h->mode == FE_EVAL_FACTORED ? kTileCostFactored : kTileCostDirect;
   int best = 0; double best_cost = 1e300;
   for (int t = 0; t < kNumTiles; ++t) {
     const double padded = (double)((nh + kTiles[t].th - 1) / kTiles[t].th * kTiles[t].th) *
                           (double)((nd + kTiles[t].td - 1) / kTiles[t].td * kTiles[t].td);
-    // sqrt + dispersion overhead per evaluation shrinks with TH: mild preference for tall tiles
-    const double cost = padded * (1.0 + 0.28 / kTiles[t].th);
+    const double cost = padded * cost_tab[t];          // padded (clamped duplicate) terms are still evaluated
     if (cost < best_cost * (1.0 - 1e-12)) { best_cost = cost; best = t; }
   }
   return best;
@@ -329,6 +334,8 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     FE_CUDA(cudaGetLastError());
     h->launches++;
   }
+  h->last_info[0] = TH; h->last_info[1] = TD; h->last_info[2] = P.ksplit; h->last_info[3] = (int32_t)grid_ll;
+  h->last_info[4] = h->mode; h->last_info[5] = P.rows_per_chunk;
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
   FE_CUDA(launch_ksum(tile, h->nb, h->p.form_factor, h->mode, (int)grid_ll, st, P));
   h->launches++;
@@ -494,6 +501,12 @@ int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
   FE_CUDA(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
   if (ksum_ms) *ksum_ms = ms;
   if (band_evals) *band_evals = h->last_band_evals;
+  return FE_OK;
+}
+
+int fe_get_last_launch_info(fe_handle* h, int32_t* info6) {
+  if (!h || !info6) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+  for (int i = 0; i < 6; ++i) info6[i] = h->last_info[i];
   return FE_OK;
 }
 

@@ -17,7 +17,7 @@ FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED = 0, 1, 2
 
 EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_scan_host",
-           "fe_enable_timing", "fe_get_timing", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info",
+           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
 
@@ -63,6 +63,7 @@ def lib():
     L.fe_enable_timing.argtypes = [vp, C.c_int32]
     L.fe_get_timing.argtypes = [vp, C.POINTER(C.c_float), dp]
     L.fe_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.fe_get_last_launch_info.argtypes = [vp, ip]
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
     L.fe_fp64_peak_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_float), dp, vp]
@@ -165,6 +166,11 @@ class FreeEnergy:
         ms, be = C.c_float(), C.c_double()
         _check(lib().fe_get_timing(self._h, C.byref(ms), C.byref(be)))
         return ms.value, be.value
+
+    def last_launch_info(self):
+        a = (C.c_int32 * 6)()
+        _check(lib().fe_get_last_launch_info(self._h, a))
+        return dict(th=a[0], td=a[1], ksplit=a[2], grid=a[3], mode=a[4], rows_per_chunk=a[5])
 
     def launch_count(self):
         n = C.c_int64()
