@@ -246,23 +246,44 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
                     const double* delta, int32_t nd, double* omega_dev, cudaStream_t st) {
   const int N = h->N;
   // ---- stage lists: [q (2nq) | h (nh) | delta^2 (nd)] ----
-  const size_t nlist = (size_t)2 * nq + nh + nd;
+  const int tile = choose_tile(h, nh, nd);
+  const int TH = kTiles[tile].th, TD = kTiles[tile].td;
+  const int ntile_h = (nh + TH - 1) / TH;
+  const int hstride = htile_stride(TH);
+  const size_t nlist = (size_t)2 * nq + nh + nd + (size_t)ntile_h * hstride;
   double *hs, *ds; StageSlot* slot;
   int rc = stage_lists(h, nlist, st, &hs, &ds, &slot);
   if (rc) return rc;
   memcpy(hs, q_xy, sizeof(double) * 2 * nq);
   memcpy(hs + 2 * nq, h_list, sizeof(double) * nh);
   for (int i = 0; i < nd; ++i) hs[2 * nq + nh + i] = delta[i] * delta[i];
+  {
+    // per-h-tile table of the factored kernel (ratios e^{-+(h_i - h_0)/T} in long double)
+    double* ht = hs + 2 * nq + nh + nd;
+    for (int t = 0; t < ntile_h; ++t, ht += hstride) {
+      const double h0 = h_list[t * TH];
+      double hmin = h0, hmax = h0;
+      for (int i = 0; i < TH; ++i) {
+        const double hi = h_list[(t * TH + i < nh) ? t * TH + i : nh - 1];
+        hmin = fmin(hmin, hi); hmax = fmax(hmax, hi);
+        const long double y = ((long double)hi - (long double)h0) / (long double)h->T;
+        ht[4 + i] = (double)expl(-y);
+        const long double ri = expl(y);
+        ht[4 + TH + i] = (ri < 1.0e301L) ? (double)ri : 1.0e301;
+      }
+      ht[0] = h0; ht[1] = hmin; ht[2] = hmax;
+      ht[3] = ((hmax - hmin) <= 600.0 * h->T) ? 1.0 : 0.0;
+    }
+  }
   FE_CUDA(cudaMemcpyAsync(ds, hs, nlist * sizeof(double), cudaMemcpyHostToDevice, st));
   FE_CUDA(cudaEventRecord(slot->ev, st));
   slot->pending = true;
   const double* d_q = ds;
   const double* d_h = ds + 2 * nq;
   const double* d_d2 = ds + 2 * nq + nh;
+  const double* d_htile = ds + 2 * nq + nh + nd;
 
   // ---- geometry ----
-  const int tile = choose_tile(h, nh, nd);
-  const int TH = kTiles[tile].th, TD = kTiles[tile].td;
   KsumParams P;
   P.mc = make_consts(h->p);
   P.T = h->T; P.neg_beta = -1.0 / h->T; P.window = 37.0 * h->T;
@@ -317,7 +338,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   nschunk = (N + srpc - 1) / srpc;
   if ((rc = ensure(h->d_spart, h->spart_cap, (size_t)nq * nschunk))) return rc;
 
-  P.coltab = h->d_coltab; P.rowtab = h->d_rowtab; P.h = d_h; P.d2 = d_d2; P.tabs = h->d_tabs;
+  P.coltab = h->d_coltab; P.rowtab = h->d_rowtab; P.h = d_h; P.d2 = d_d2; P.htile = d_htile; P.tabs = h->d_tabs;
   P.partial = h->d_partial;
 
   // ---- K0 trig, KS constant sum, K1 k-sum, K2 finish ----

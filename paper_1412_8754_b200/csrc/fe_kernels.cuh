@@ -46,6 +46,7 @@ struct KsumParams {
   const double4* rowtab;               // [nq][N] {cos ky, sin ky, cos(ky-qy), sin(ky-qy)}
   const double* h;                     // [nh]
   const double* d2;                    // [nd]  Delta^2
+  const double* htile;                 // [ntile_h][4 + 2 TH] per-h-tile table of the factored kernel
   const MathTabs* tabs;                // global copy of the exp/log tables
   double* partial;                     // [ksplit][nq*nh*nd]
 };
@@ -294,8 +295,7 @@ struct FactoredConsts {       // per-temperature constants of the extended-range
 __device__ __forceinline__ double exp_mant(double x, double t, const FactoredConsts& fc, const double* __restrict__ tab256) {
   const double MAGIC = 6755399441055744.0;        // 1.5 * 2^52
   const double nf = t - MAGIC;
-  double r = fma(nf, -fc.c2hi, x);
-  r = fma(nf, -fc.c2lo, r);
+  const double r = fma(nf, -fc.c2hi, x);          // single constant: the lo part would change ln Z by < ulp(x)/(2T) * T
   double p = fma(r, fc.b4, fc.b3);
   p = fma(p, r, fc.b2);
   p = fma(p, r, fc.b1);
@@ -326,15 +326,20 @@ __device__ __forceinline__ double scale2(double m, int shift) {   // m * 2^shift
   return __hiloint2double(__double2hiint(m) + (s << 20), __double2loint(m));
 }
 
+// Per-h-tile table (host, long double): [h0, hmin, hmax, hrec_ok, rho[TH], rhoinv[TH]] with
+// rho_i = exp(-(h_i - h0)/T), rhoinv_i = exp(+(h_i - h0)/T) (clamped to 2^1000), hrec_ok = (hmax - hmin <= 600 T).
+__host__ __device__ constexpr int htile_stride(int TH) { return 4 + 2 * TH; }
+
 template <int NB, int FORM, int TH, int TD>
 __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
   __shared__ double tab256[256];
-  __shared__ double hv_s[TH], d2v_s[TD];
+  __shared__ double hv_s[TH], rho_s[TH], rhoinv_s[TH], d2v_s[TD], hinfo_s[4];
   __shared__ int accE_s[TH * TD][kThreads];        // robust-path exponent sums, [pair][thread]
   __shared__ double red[kWarps][TH * TD];
   for (int i = threadIdx.x; i < 256; i += kThreads) tab256[i] = P.tabs->exp2_j256[i];
+  int* const myE = &accE_s[0][threadIdx.x];
 #pragma unroll
-  for (int pq = 0; pq < TH * TD; ++pq) accE_s[pq][threadIdx.x] = 0;
+  for (int pq = 0; pq < TH * TD; ++pq) myE[pq * kThreads] = 0;
 
   int b = blockIdx.x;
   const int chunk = b % P.ksplit;  b /= P.ksplit;
@@ -349,8 +354,16 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
   const int by = kThreads >> P.bx_log2;
   const bool valid = col < P.N;
 
-  if (threadIdx.x < TH) hv_s[threadIdx.x] = P.h[min(th * TH + (int)threadIdx.x, P.nh - 1)];
-  if (threadIdx.x < TD) d2v_s[threadIdx.x] = P.d2[min(td * TD + (int)threadIdx.x, P.nd - 1)];
+  {
+    const double* ht = P.htile + (size_t)th * htile_stride(TH);
+    if (threadIdx.x < 4) hinfo_s[threadIdx.x] = ht[threadIdx.x];
+    if (threadIdx.x < TH) {
+      hv_s[threadIdx.x] = P.h[min(th * TH + (int)threadIdx.x, P.nh - 1)];
+      rho_s[threadIdx.x] = ht[4 + threadIdx.x];
+      rhoinv_s[threadIdx.x] = ht[4 + TH + threadIdx.x];
+    }
+    if (threadIdx.x < TD) d2v_s[threadIdx.x] = P.d2[min(td * TD + (int)threadIdx.x, P.nd - 1)];
+  }
 
   double accP[TH][TD];
 #pragma unroll
@@ -368,6 +381,8 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
     const double4* rt = P.rowtab + (size_t)iq * P.N;
     const int r0 = rs * P.rows_per_chunk;
     const int r1 = min(P.N, r0 + P.rows_per_chunk);
+    const double hmin = hinfo_s[1], hmax = hinfo_s[2];
+    const bool hrec = hinfo_s[3] != 0.0;
 
     for (int rb = r0 + rsub; rb < r1; rb += by * kRenorm) {
       const int rend = min(r1, rb + by * kRenorm);
@@ -392,10 +407,10 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
           const double d0 = (e == 0) ? dA[0] : dA[NB - 1];
           const double s2 = s * s;
 
-          // ---- pass 1: binary exponents of all A_j, B_i ----
+          // ---- A_j = 2cosh(R_j/T), j < TD: four independent chains ----
           double mA[TD];
-          int eA[TD], eB[TH];
-          int emaxA = 0, eminA = 0x7fffffff, emaxB = 0, eminB = 0x7fffffff;
+          int eA[TD];
+          int emaxA = 0, eminA = 0x7fffffff;
 #pragma unroll
           for (int j = 0; j < TD; ++j) {
             const double R = sqrt(fma(d2v_s[j], g2, s2));                  // Eq. 4 radicand
@@ -408,41 +423,70 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
 #pragma unroll
             for (int j = 0; j < TD; ++j) mA[j] = cosh_fix(mA[j], eA[j]);
           }
-#pragma unroll
-          for (int i = 0; i < TH; ++i) {
-            const double t = fma(fabs(d0 - hv_s[i]), fc.c1, MAGIC);
-            eB[i] = exp_k(t);
-            emaxB = max(emaxB, eB[i]); eminB = min(eminB, eB[i]);
-          }
-          const int Eref = max(emaxA, emaxB);
-          const bool fixB = __any_sync(wmask, eminB < 28);
-          const bool fast = __all_sync(wmask, max(eminA, eminB) >= Eref - kSpread);
+
+          // ---- exponent bounds of the B_i from the tile's h range: y_i = d0 - h_i lies in [dlo, dhi] ----
+          const double dlo = d0 - hmax, dhi = d0 - hmin;
+          const double ymax = fmax(fabs(dlo), fabs(dhi));
+          const double ymin = fmax(0.0, fmax(dlo, -dhi));                 // distance of 0 from [dlo, dhi]
+          const int eBhi = exp_k(fma(ymax, fc.c1, MAGIC)) + 1;            // B_i < 2^(eBhi + 1)
+          const int eBlo = exp_k(fma(ymin, fc.c1, MAGIC));                // B_i >= 2^eBlo
+          const int Eref = max(emaxA, eBhi);
+          const bool fast = __all_sync(wmask, max(eminA, eBlo) >= Eref - kSpread);
 
           if (fast) {
             accEc += Eref;
-            double Ap[TD];
+            double Ap[TD], Bp[TH];
 #pragma unroll
             for (int j = 0; j < TD; ++j) Ap[j] = scale2(mA[j], eA[j] - Eref);
+            if (hrec) {
+              // one exponential for the tile: e^{+-y_0/T}; the others by the host-made ratios rho_i
+              const double y0 = d0 - hv_s[0];
+              const double ay = fabs(y0);
+              const double t = fma(ay, fc.c1, MAGIC);
+              const int eb = exp_k(t);
+              const double mb = exp_mant(ay, t, fc, tab256);
+              double rc;
+              asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(mb));
+              double er = fma(-mb, rc, 1.0);
+              rc = fma(rc, er, rc);
+              er = fma(-mb, rc, 1.0);
+              rc = fma(rc, er, rc);
+              const double big = scale2(mb, eb - Eref);                    // e^{+|y0|/T} 2^-Eref
+              const double sml = scale2(rc, -eb - Eref);                   // e^{-|y0|/T} 2^-Eref
+              const double P0 = (y0 >= 0.0) ? big : sml;                   // e^{+y0/T} 2^-Eref
+              const double M0 = (y0 >= 0.0) ? sml : big;                   // e^{-y0/T} 2^-Eref
 #pragma unroll
-            for (int i = 0; i < TH; ++i) {
-              const double ad = fabs(d0 - hv_s[i]);
-              double mB = exp_mant(ad, fma(ad, fc.c1, MAGIC), fc, tab256);
-              if (fixB) mB = cosh_fix(mB, eB[i]);
-              const double Bp = scale2(mB, eB[i] - Eref);
+              for (int i = 0; i < TH; ++i) Bp[i] = fma(M0, rhoinv_s[i], P0 * rho_s[i]);
+            } else {
+              const bool fixB = __any_sync(wmask, eBlo < 28);
 #pragma unroll
-              for (int j = 0; j < TD; ++j) accP[i][j] *= (Ap[j] + Bp);
+              for (int i = 0; i < TH; ++i) {
+                const double ad = fabs(d0 - hv_s[i]);
+                const double t = fma(ad, fc.c1, MAGIC);
+                const int eb = exp_k(t);
+                double mB = exp_mant(ad, t, fc, tab256);
+                if (fixB) mB = cosh_fix(mB, eb);
+                Bp[i] = scale2(mB, eb - Eref);
+              }
             }
+#pragma unroll
+            for (int i = 0; i < TH; ++i)
+#pragma unroll
+              for (int j = 0; j < TD; ++j) accP[i][j] *= (Ap[j] + Bp[i]);
           } else {
+            const bool fixB = __any_sync(wmask, eBlo < 28);
 #pragma unroll
             for (int i = 0; i < TH; ++i) {
               const double ad = fabs(d0 - hv_s[i]);
-              double mB = exp_mant(ad, fma(ad, fc.c1, MAGIC), fc, tab256);
-              if (fixB) mB = cosh_fix(mB, eB[i]);
+              const double t = fma(ad, fc.c1, MAGIC);
+              const int eb = exp_k(t);
+              double mB = exp_mant(ad, t, fc, tab256);
+              if (fixB) mB = cosh_fix(mB, eb);
 #pragma unroll
               for (int j = 0; j < TD; ++j) {
-                const int E = max(eA[j], eB[i]);
-                accP[i][j] *= (scale2(mA[j], eA[j] - E) + scale2(mB, eB[i] - E));
-                accE_s[i * TD + j][threadIdx.x] += E;
+                const int E = max(eA[j], eb);
+                accP[i][j] *= (scale2(mA[j], eA[j] - E) + scale2(mB, eb - E));
+                myE[(i * TD + j) * kThreads] += E;
               }
             }
           }
@@ -455,7 +499,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
         for (int j = 0; j < TD; ++j) {
           const int hi = __double2hiint(accP[i][j]);
           const int ex = (hi >> 20) - 1023;
-          accE_s[i * TD + j][threadIdx.x] += ex;
+          myE[(i * TD + j) * kThreads] += ex;
           accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
         }
     }
@@ -468,7 +512,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
   for (int i = 0; i < TH; ++i)
 #pragma unroll
     for (int j = 0; j < TD; ++j) {
-      const double ed = (double)accEc + (double)accE_s[i * TD + j][threadIdx.x];
+      const double ed = (double)accEc + (double)myE[(i * TD + j) * kThreads];
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(accP[i][j])));
       const double v = warp_sum(P.T * lnz);
       if (lane == 0) red[warp][i * TD + j] = v;
