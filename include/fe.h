@@ -134,6 +134,9 @@ int fe_get_launch_count(fe_handle* h, int64_t* launches);
  * target_blocks: minimum number of thread blocks K1 should be split into (0 = auto).               */
 int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks);
 int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past the end of the table */
+/* Test hook for FE_EVAL_FACTORED: bit 0 = always take the robust per-pair path, bit 1 = never use the per-tile
+ * h recurrence.  Results are the same sums; only the code path changes (lets tests cover each path).       */
+int fe_set_debug_flags(fe_handle* h, int32_t flags);
 
 /* FP64 DFMA-chain microbenchmark on the current device (register-resident, no memory traffic):
  * runs `blocks` blocks of 256 threads, each thread `iters` x 16 dependent-chain-interleaved DFMAs,

@@ -49,6 +49,7 @@ struct fe_handle {
   int32_t mode = FE_EVAL_FACTORED;
   int32_t tile = 0;            // 0 = auto, else 1 + index
   int32_t target_blocks = 0;   // 0 = auto
+  int32_t debug_flags = 0;
   int device = 0;
   int sm_count = 148;
   int nb = 1;
@@ -258,21 +259,25 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   memcpy(hs + 2 * nq, h_list, sizeof(double) * nh);
   for (int i = 0; i < nd; ++i) hs[2 * nq + nh + i] = delta[i] * delta[i];
   {
-    // per-h-tile table of the factored kernel (ratios e^{-+(h_i - h_0)/T} in long double)
+    // per-h-tile table of the factored kernel (fe_kernels.cuh "Per-h-tile table"), in long double
     double* ht = hs + 2 * nq + nh + nd;
+    const long double Tl = (long double)h->T;
     for (int t = 0; t < ntile_h; ++t, ht += hstride) {
-      const double h0 = h_list[t * TH];
-      double hmin = h0, hmax = h0;
+      double hmin = h_list[t * TH], hmax = hmin;
       for (int i = 0; i < TH; ++i) {
         const double hi = h_list[(t * TH + i < nh) ? t * TH + i : nh - 1];
         hmin = fmin(hmin, hi); hmax = fmax(hmax, hi);
-        const long double y = ((long double)hi - (long double)h0) / (long double)h->T;
-        ht[4 + i] = (double)expl(-y);
-        const long double ri = expl(y);
-        ht[4 + TH + i] = (ri < 1.0e301L) ? (double)ri : 1.0e301;
       }
-      ht[0] = h0; ht[1] = hmin; ht[2] = hmax;
-      ht[3] = ((hmax - hmin) <= 600.0 * h->T) ? 1.0 : 0.0;
+      for (int i = 0; i < TH; ++i) {
+        const double hi = h_list[(t * TH + i < nh) ? t * TH + i : nh - 1];
+        ht[4 + i] = (double)expl(-((long double)hi - (long double)hmin) / Tl);
+        ht[4 + TH + i] = (double)expl(-((long double)hmax - (long double)hi) / Tl);
+      }
+      const long double l2 = ((long double)hmax - (long double)hmin) / Tl * 1.442695040888963407359924681001892137L;
+      const long double fl = floorl(l2);
+      ht[0] = hmin; ht[1] = hmax;
+      ht[2] = (double)exp2l(l2 - fl);              // mC in [1, 2)
+      ht[3] = (double)fl;                          // eC (< 2^31: max|h|/T < 1e9 is enforced below)
     }
   }
   FE_CUDA(cudaMemcpyAsync(ds, hs, nlist * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -288,6 +293,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   P.mc = make_consts(h->p);
   P.T = h->T; P.neg_beta = -1.0 / h->T; P.window = 37.0 * h->T;
   P.N = N; P.nq = nq; P.nh = nh; P.nd = nd;
+  P.debug_flags = h->debug_flags;
   P.ntile_h = (nh + TH - 1) / TH;
   P.ntile_d = (nd + TD - 1) / TD;
   int bxl = 8;                                   // 256 columns per block when N allows it
@@ -449,6 +455,13 @@ int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks) {
   if (tile < 0 || tile > kNumTiles || target_blocks < 0) {
     snprintf(g_errbuf, sizeof g_errbuf, "tile must be in [0, %d], target_blocks >= 0", kNumTiles); return FE_EINVAL; }
   h->tile = tile; h->target_blocks = target_blocks;
+  return FE_OK;
+}
+
+int fe_set_debug_flags(fe_handle* h, int32_t flags) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (flags < 0 || flags > 3) { snprintf(g_errbuf, sizeof g_errbuf, "flags must be in [0, 3]"); return FE_EINVAL; }
+  h->debug_flags = flags;
   return FE_OK;
 }
 

@@ -42,6 +42,7 @@ struct KsumParams {
   int32_t ntile_h, ntile_d;
   int32_t bx_log2;                     // block = 2^bx_log2 columns x (256 >> bx_log2) row lanes
   int32_t ncg, nrs, rows_per_chunk, ksplit;   // column groups, row splits; ksplit = ncg * nrs
+  int32_t debug_flags;                 // bit 0: never take the fast path, bit 1: never use the h recurrence (tests)
   const double4* coltab;               // [nq][N] {cos kx, sin kx, cos(kx-qx), sin(kx-qx)}
   const double4* rowtab;               // [nq][N] {cos ky, sin ky, cos(ky-qy), sin(ky-qy)}
   const double* h;                     // [nh]
@@ -282,8 +283,8 @@ __global__ void __launch_bounds__(kThreads) fe_ksum_kernel(const KsumParams P) {
 //        shared memory ([pair][thread], conflict-free).
 // accP is renormalised every kRenorm rows (its exponent moved into accEc ... see code).  (DESIGN.md "K1f".)
 // ---------------------------------------------------------------------------------------------------
-constexpr int kRenorm = 32;   // rows between renormalisations: <= 64 factors in [2^-9, 5.2): 2^-576 .. 2^153
-constexpr int kSpread = 8;    // fast path: all pair exponents within 2^-8 of the tile maximum
+constexpr int kSpread = 900;       // fast path: every pair within 2^-900 of the tile maximum (all terms normal doubles)
+constexpr int kDriftLimit = 1000;  // renormalise accP before its exponent can have drifted by more than this
 
 struct FactoredConsts {       // per-temperature constants of the extended-range exponential (host, long double)
   double c1;                  // 256 / (T ln2):        n = rint(x c1)
@@ -321,19 +322,22 @@ __device__ __forceinline__ int exp_k(double t) {  // n >> 8 from the 52-bit mant
   return __funnelshift_r(__double2loint(t), __double2hiint(t), 8);
 }
 
-__device__ __forceinline__ double scale2(double m, int shift) {   // m * 2^shift, shift <= 0, flushed at 2^-1000
+__device__ __forceinline__ double scale2(double m, int shift) {   // m * 2^shift (shift <= ~2); exactly 0 below 2^-1000
   const int s = max(shift, -1000);
-  return __hiloint2double(__double2hiint(m) + (s << 20), __double2loint(m));
+  const double v = __hiloint2double(__double2hiint(m) + (s << 20), __double2loint(m));
+  return shift < -1000 ? 0.0 : v;
 }
 
-// Per-h-tile table (host, long double): [h0, hmin, hmax, hrec_ok, rho[TH], rhoinv[TH]] with
-// rho_i = exp(-(h_i - h0)/T), rhoinv_i = exp(+(h_i - h0)/T) (clamped to 2^1000), hrec_ok = (hmax - hmin <= 600 T).
+// Per-h-tile table (host, long double): [hmin, hmax, mC, eC, rho[TH], sig[TH]] with
+//   rho_i = exp(-(h_i - hmin)/T) <= 1,  sig_i = exp(-(hmax - h_i)/T) <= 1,  C = exp((hmax - hmin)/T) = mC 2^eC.
+// Then e^{(d0-h_i)/T} = e^{(d0-hmin)/T} rho_i and e^{-(d0-h_i)/T} = [C / e^{(d0-hmin)/T}] sig_i: both ratios are <= 1,
+// so a flushed (negligible) reference term can never be amplified back into significance.
 __host__ __device__ constexpr int htile_stride(int TH) { return 4 + 2 * TH; }
 
 template <int NB, int FORM, int TH, int TD>
 __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
   __shared__ double tab256[256];
-  __shared__ double hv_s[TH], rho_s[TH], rhoinv_s[TH], d2v_s[TD], hinfo_s[4];
+  __shared__ double hv_s[TH], rho_s[TH], sig_s[TH], d2v_s[TD], hinfo_s[4];
   __shared__ int accE_s[TH * TD][kThreads];        // robust-path exponent sums, [pair][thread]
   __shared__ double red[kWarps][TH * TD];
   for (int i = threadIdx.x; i < 256; i += kThreads) tab256[i] = P.tabs->exp2_j256[i];
@@ -360,7 +364,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
     if (threadIdx.x < TH) {
       hv_s[threadIdx.x] = P.h[min(th * TH + (int)threadIdx.x, P.nh - 1)];
       rho_s[threadIdx.x] = ht[4 + threadIdx.x];
-      rhoinv_s[threadIdx.x] = ht[4 + TH + threadIdx.x];
+      sig_s[threadIdx.x] = ht[4 + TH + threadIdx.x];
     }
     if (threadIdx.x < TD) d2v_s[threadIdx.x] = P.d2[min(td * TD + (int)threadIdx.x, P.nd - 1)];
   }
@@ -381,12 +385,14 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
     const double4* rt = P.rowtab + (size_t)iq * P.N;
     const int r0 = rs * P.rows_per_chunk;
     const int r1 = min(P.N, r0 + P.rows_per_chunk);
-    const double hmin = hinfo_s[1], hmax = hinfo_s[2];
-    const bool hrec = hinfo_s[3] != 0.0;
+    const double hmin = hinfo_s[0], hmax = hinfo_s[1], mC = hinfo_s[2];
+    const int eC = (int)hinfo_s[3];
+    const bool hrec = !(P.debug_flags & 2);
+    const int spread_limit = (P.debug_flags & 1) ? -1 : kSpread;
 
-    for (int rb = r0 + rsub; rb < r1; rb += by * kRenorm) {
-      const int rend = min(r1, rb + by * kRenorm);
-      for (int r = rb; r < rend; r += by) {
+    int drift = 0;                                 // bound on |log2| accumulated by any accP since its last renormalisation
+    for (int r = r0 + rsub; r < r1; r += by) {
+      {
         const double4 rr = rt[r];
         double Ek[NB], Eq[NB];
         band_energies<NB>(P.mc, ct.x, ct.y, rr.x, rr.y, Ek);
@@ -431,7 +437,24 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
           const int eBhi = exp_k(fma(ymax, fc.c1, MAGIC)) + 1;            // B_i < 2^(eBhi + 1)
           const int eBlo = exp_k(fma(ymin, fc.c1, MAGIC));                // B_i >= 2^eBlo
           const int Eref = max(emaxA, eBhi);
-          const bool fast = __all_sync(wmask, max(eminA, eBlo) >= Eref - kSpread);
+          const int spread = Eref - max(eminA, eBlo);                      // every pair sum is in [2^-spread, 2^3.4)
+          const bool fast = __all_sync(wmask, spread <= spread_limit);
+
+          // a factor changes log2(accP) by at most max(spread, 4): renormalise before the budget is exceeded
+          const int step = fast ? max(spread, 4) : 4;
+          if (__any_sync(wmask, drift + step > kDriftLimit)) {
+#pragma unroll
+            for (int i = 0; i < TH; ++i)
+#pragma unroll
+              for (int j = 0; j < TD; ++j) {
+                const int hi = __double2hiint(accP[i][j]);
+                const int ex = (hi >> 20) - 1023;
+                myE[(i * TD + j) * kThreads] += ex;
+                accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
+              }
+            drift = 0;
+          }
+          drift += step;
 
           if (fast) {
             accEc += Eref;
@@ -439,9 +462,9 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
 #pragma unroll
             for (int j = 0; j < TD; ++j) Ap[j] = scale2(mA[j], eA[j] - Eref);
             if (hrec) {
-              // one exponential for the tile: e^{+-y_0/T}; the others by the host-made ratios rho_i
-              const double y0 = d0 - hv_s[0];
-              const double ay = fabs(y0);
+              // one exponential for the whole h tile: Pm = e^{(d0-hmin)/T} (the largest e^{+y_i/T}) and
+              // Mm = C / Pm = e^{(hmax-d0)/T} (the largest e^{-y_i/T}); the others by the host-made ratios <= 1
+              const double ay = fabs(dhi);
               const double t = fma(ay, fc.c1, MAGIC);
               const int eb = exp_k(t);
               const double mb = exp_mant(ay, t, fc, tab256);
@@ -451,12 +474,12 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
               rc = fma(rc, er, rc);
               er = fma(-mb, rc, 1.0);
               rc = fma(rc, er, rc);
-              const double big = scale2(mb, eb - Eref);                    // e^{+|y0|/T} 2^-Eref
-              const double sml = scale2(rc, -eb - Eref);                   // e^{-|y0|/T} 2^-Eref
-              const double P0 = (y0 >= 0.0) ? big : sml;                   // e^{+y0/T} 2^-Eref
-              const double M0 = (y0 >= 0.0) ? sml : big;                   // e^{-y0/T} 2^-Eref
+              const bool pos = dhi >= 0.0;
+              const int pe = pos ? eb : -eb;
+              const double P0 = scale2(pos ? mb : rc, pe - Eref);                 // e^{(d0-hmin)/T} 2^-Eref
+              const double M0 = scale2((pos ? rc : mb) * mC, eC - pe - Eref);     // e^{(hmax-d0)/T} 2^-Eref
 #pragma unroll
-              for (int i = 0; i < TH; ++i) Bp[i] = fma(M0, rhoinv_s[i], P0 * rho_s[i]);
+              for (int i = 0; i < TH; ++i) Bp[i] = fma(M0, sig_s[i], P0 * rho_s[i]);
             } else {
               const bool fixB = __any_sync(wmask, eBlo < 28);
 #pragma unroll
@@ -492,17 +515,17 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
           }
         }
       }
-      // renormalise: move the binary exponent of each running product into the integer sums
-#pragma unroll
-      for (int i = 0; i < TH; ++i)
-#pragma unroll
-        for (int j = 0; j < TD; ++j) {
-          const int hi = __double2hiint(accP[i][j]);
-          const int ex = (hi >> 20) - 1023;
-          myE[(i * TD + j) * kThreads] += ex;
-          accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
-        }
     }
+    // final renormalisation so that ln(accP) below sees a mantissa in [1, 2)
+#pragma unroll
+    for (int i = 0; i < TH; ++i)
+#pragma unroll
+      for (int j = 0; j < TD; ++j) {
+        const int hi = __double2hiint(accP[i][j]);
+        const int ex = (hi >> 20) - 1023;
+        myE[(i * TD + j) * kThreads] += ex;
+        accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
+      }
   }
 
   // per-thread P = T (ln2 * exponent sum + ln accP), then the same fixed-order reduction as K1

@@ -17,7 +17,7 @@ FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED = 0, 1, 2
 
 EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_scan_host",
-           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info",
+           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
 
@@ -66,6 +66,7 @@ def lib():
     L.fe_get_last_launch_info.argtypes = [vp, ip]
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
+    L.fe_set_debug_flags.argtypes = [vp, C.c_int32]
     L.fe_fp64_peak_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_float), dp, vp]
     L.fe_debug_math.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp]
     L.fe_destroy.argtypes = [vp]
@@ -157,6 +158,9 @@ class FreeEnergy:
 
     def set_tuning(self, tile=0, target_blocks=0):
         _check(lib().fe_set_tuning(self._h, int(tile), int(target_blocks)))
+
+    def set_debug_flags(self, flags):
+        _check(lib().fe_set_debug_flags(self._h, int(flags)))
 
     def enable_timing(self, on=True):
         _check(lib().fe_enable_timing(self._h, 1 if on else 0))

@@ -20,11 +20,12 @@ GAP = 1e-10
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
-def run_gpu(fe, w, T, mode=0, tile=0, target_blocks=0):
+def run_gpu(fe, w, T, mode=0, tile=0, target_blocks=0, flags=0):
     import torch
     with fe.FreeEnergy(w.params, w.N, T) as F:
         F.set_eval_mode(mode)
         F.set_tuning(tile, target_blocks)
+        F.set_debug_flags(flags)
         om = F.omega_grid(w.q, w.h, w.delta)
         idx, ds, os_ = F.argmin(om, w.delta)
         torch.cuda.synchronize()
@@ -97,6 +98,29 @@ def test_ragged_one_band(fe, oracle, tile):
     w = W.ragged(seed=11, N=301, nq=2, nh=3, nd=9, model=W.MODEL_ONE_BAND)
     parity(fe, oracle, w, w.T[0], tile=tile)
     parity(fe, oracle, w, 0.3, tile=tile)                 # hot: thermal part is O(1) of Omega
+
+
+@pytest.mark.parametrize("flags", [0, 1, 2, 3])
+def test_factored_kernel_every_code_path(fe, oracle, flags):
+    """FE_EVAL_FACTORED has a fast path (with / without the per-tile h recurrence) and a robust per-pair path chosen
+    per warp; force each one on workloads that normally take another and compare all with the oracle."""
+    for w, temps in ((W.ragged(seed=23, N=70, nq=2, nh=11, nd=9), (0.004, 0.05, 1e-4)),
+                     (W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=16, nd=32), (0.001, 0.01)),
+                     (W.ragged(seed=29, N=50, nq=1, nh=9, nd=5, model=W.MODEL_ONE_BAND), (0.02,))):
+        for T in temps:
+            for tile in (1, 2):
+                parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED, tile=tile, flags=flags)
+
+
+def test_factored_extreme_spreads(fe, oracle):
+    """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
+    the spread exceeds 900 binades (robust path taken on its own)."""
+    p = W.model_params(U=4.0)
+    h = np.array([0.0, 0.29, 0.01, 0.7, 0.3, 0.02, 1.5, 0.11])           # unsorted, wide
+    d = np.array([0.0, 0.4, 0.05, 1.0, 0.2])
+    w = W.Workload("wide_h", p, 40, (0.001,), np.array([[0.3, 0.1], [0.0, 0.0]]), h, d)
+    for T in (0.001, 2e-4, 3e-5, 0.2):
+        parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED)
 
 
 def test_ksplit_variants_agree_and_match(fe, oracle):
