@@ -52,6 +52,23 @@ struct KsumParams {
   double* partial;                     // [ksplit][nq*nh*nd]
 };
 
+// Branch-free sqrt for normal x > 0 (callers add 1e-300 to the radicand so x = 0 cannot occur): rsqrt seed (MUFU),
+// two coupled Newton steps and one residual correction; <= 1 ulp, no slow path, so independent chains interleave.
+__device__ __forceinline__ double sqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y;            // ~ sqrt(x)
+  double h = 0.5 * y;          // ~ 1 / (2 sqrt(x))
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  const double d = fma(-g, g, x);
+  return fma(d, h, g);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Band energies at one k from its four trig values (S2).  E[0] = E_+, E[1] = E_- (A.4).
 // ---------------------------------------------------------------------------------------------------
@@ -65,7 +82,7 @@ __device__ __forceinline__ void band_energies(const ModelConsts& mc, double cx, 
     const double avg = fma(mc.t3x4, cx * cy, mc.tp * (cx + cy));
     const double dif = mc.tm * (cx - cy);
     const double off = mc.t4x4 * (sx * sy);
-    const double rad = sqrt(fma(dif, dif, off * off));
+    const double rad = sqrt_pos(fma(dif, dif, fma(off, off, 1e-300)));
     E[0] = avg + rad;
     E[NB - 1] = avg - rad;
   }
@@ -411,15 +428,28 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
           if (!((P.mc.band_mask >> e) & 1)) continue;
           const double s = (e == 0) ? sA[0] : sA[NB - 1];
           const double d0 = (e == 0) ? dA[0] : dA[NB - 1];
-          const double s2 = s * s;
+          const double s2 = fma(s, s, 1e-300);                            // keeps the radicand > 0
 
-          // ---- A_j = 2cosh(R_j/T), j < TD: four independent chains ----
+          // ---- A_j = 2cosh(R_j/T), j < TD, and the one exponential of the h tile: TD + 1 independent chains ----
+          const double dlo = d0 - hmax, dhi = d0 - hmin;                  // y_i = d0 - h_i lies in [dlo, dhi]
+          const double ayB = fabs(dhi);
+          const double tB = fma(ayB, fc.c1, MAGIC);
+          const int ebB = exp_k(tB);
+          const double mbB = exp_mant(ayB, tB, fc, tab256);               // e^{|d0-hmin|/T} = mbB 2^ebB
+          double rcB;
+          asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rcB) : "d"(mbB));
+          {
+            double er = fma(-mbB, rcB, 1.0);
+            rcB = fma(rcB, er, rcB);
+            er = fma(-mbB, rcB, 1.0);
+            rcB = fma(rcB, er, rcB);                                       // 1/mbB
+          }
           double mA[TD];
           int eA[TD];
           int emaxA = 0, eminA = 0x7fffffff;
 #pragma unroll
           for (int j = 0; j < TD; ++j) {
-            const double R = sqrt(fma(d2v_s[j], g2, s2));                  // Eq. 4 radicand
+            const double R = sqrt_pos(fma(d2v_s[j], g2, s2));              // Eq. 4 radicand
             const double t = fma(R, fc.c1, MAGIC);
             eA[j] = exp_k(t);
             mA[j] = exp_mant(R, t, fc, tab256);
@@ -431,7 +461,6 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
           }
 
           // ---- exponent bounds of the B_i from the tile's h range: y_i = d0 - h_i lies in [dlo, dhi] ----
-          const double dlo = d0 - hmax, dhi = d0 - hmin;
           const double ymax = fmax(fabs(dlo), fabs(dhi));
           const double ymin = fmax(0.0, fmax(dlo, -dhi));                 // distance of 0 from [dlo, dhi]
           const int eBhi = exp_k(fma(ymax, fc.c1, MAGIC)) + 1;            // B_i < 2^(eBhi + 1)
@@ -462,18 +491,10 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
 #pragma unroll
             for (int j = 0; j < TD; ++j) Ap[j] = scale2(mA[j], eA[j] - Eref);
             if (hrec) {
-              // one exponential for the whole h tile: Pm = e^{(d0-hmin)/T} (the largest e^{+y_i/T}) and
-              // Mm = C / Pm = e^{(hmax-d0)/T} (the largest e^{-y_i/T}); the others by the host-made ratios <= 1
-              const double ay = fabs(dhi);
-              const double t = fma(ay, fc.c1, MAGIC);
-              const int eb = exp_k(t);
-              const double mb = exp_mant(ay, t, fc, tab256);
-              double rc;
-              asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(mb));
-              double er = fma(-mb, rc, 1.0);
-              rc = fma(rc, er, rc);
-              er = fma(-mb, rc, 1.0);
-              rc = fma(rc, er, rc);
+              // Pm = e^{(d0-hmin)/T} (the largest e^{+y_i/T}) and Mm = C / Pm = e^{(hmax-d0)/T} (the largest
+              // e^{-y_i/T}); the other h values of the tile by the host-made ratios <= 1
+              const int eb = ebB;
+              const double mb = mbB, rc = rcB;
               const bool pos = dhi >= 0.0;
               const int pe = pos ? eb : -eb;
               const double P0 = scale2(pos ? mb : rc, pe - Eref);                 // e^{(d0-hmin)/T} 2^-Eref
