@@ -41,7 +41,8 @@ def build(force: bool = False, extra=(), verbose: bool = False) -> str:
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as f:
         f.write(" ".join(cmd) + "\n" + log)
     if r.returncode != 0:
-        sys.stderr.write(log)
+        errs = [l for l in log.splitlines() if "error" in l.lower()]
+        sys.stderr.write("\n".join(errs[:20]) + "\n(full log: paper_1412_8754_b200/build_ptxas.log)\n")
         raise RuntimeError("nvcc failed")
     if verbose:
         print(log)

@@ -212,7 +212,7 @@ template <int NB, int FORM, int TH, int TD>
 cudaError_t launch_ksum_mode(int mode, int grid, cudaStream_t st, const KsumParams& P) {
   if (mode == FE_EVAL_WINDOWED)    fe_ksum_kernel<NB, FORM, TH, TD, 1><<<grid, kThreads, 0, st>>>(P);
   else if (mode == FE_EVAL_DIRECT) fe_ksum_kernel<NB, FORM, TH, TD, 0><<<grid, kThreads, 0, st>>>(P);
-  else                             fe_ksum_factored_kernel<NB, FORM, TH, TD><<<grid, kThreads, 0, st>>>(P, make_factored(P.T));
+  else                             fe_ksum_factored_kernel<NB, FORM, TH, TD><<<grid, kFThreads, 0, st>>>(P, make_factored(P.T));
   return cudaGetLastError();
 }
 
@@ -296,10 +296,12 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   P.debug_flags = h->debug_flags;
   P.ntile_h = (nh + TH - 1) / TH;
   P.ntile_d = (nd + TD - 1) / TD;
-  int bxl = 8;                                   // 256 columns per block when N allows it
+  const int bthreads = h->mode == FE_EVAL_FACTORED ? kFThreads : kThreads;
+  int bxl = 0;
+  while ((1 << bxl) < bthreads) ++bxl;           // all threads along kx when N allows it
   while (bxl > 5 && (1 << (bxl - 1)) >= N) --bxl;
   P.bx_log2 = bxl;
-  const int bx = 1 << bxl, by = kThreads >> bxl;
+  const int bx = 1 << bxl, by = bthreads >> bxl;
   P.ncg = (N + bx - 1) / bx;
   const long long ntiles = (long long)nq * P.ntile_h * P.ntile_d;
   const long long target = h->target_blocks > 0 ? h->target_blocks : (long long)h->sm_count * 2 * 24;

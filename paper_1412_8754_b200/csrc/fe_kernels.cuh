@@ -351,16 +351,26 @@ __device__ __forceinline__ double scale2(double m, int shift) {   // m * 2^shift
 // so a flushed (negligible) reference term can never be amplified back into significance.
 __host__ __device__ constexpr int htile_stride(int TH) { return 4 + 2 * TH; }
 
+// Measured on B200 (config-4 step, tile 8x4): 256 thr x 2 blocks/SM (128 regs, spills) 38.5 ms; 128 x 3 (168 regs,
+// no spills, 12 warps/SM) 35.7 ms; 128 x 4 (128 regs) 38.0 ms; 128 x 2 (191 regs) 40.4 ms; 64 x 6 35.7 ms.
+#ifndef FE_FACTORED_MINBLOCKS
+#define FE_FACTORED_MINBLOCKS 3
+#endif
+#ifndef FE_FACTORED_THREADS
+#define FE_FACTORED_THREADS 128
+#endif
+constexpr int kFThreads = FE_FACTORED_THREADS;   // threads per block of the factored kernel
+constexpr int kFWarps = kFThreads / 32;
 template <int NB, int FORM, int TH, int TD>
-__global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
+__global__ void __launch_bounds__(kFThreads, FE_FACTORED_MINBLOCKS) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
   __shared__ double tab256[256];
   __shared__ double hv_s[TH], rho_s[TH], sig_s[TH], d2v_s[TD], hinfo_s[4];
-  __shared__ int accE_s[TH * TD][kThreads];        // robust-path exponent sums, [pair][thread]
-  __shared__ double red[kWarps][TH * TD];
-  for (int i = threadIdx.x; i < 256; i += kThreads) tab256[i] = P.tabs->exp2_j256[i];
+  __shared__ int accE_s[TH * TD][kFThreads];        // robust-path exponent sums, [pair][thread]
+  __shared__ double red[kFWarps][TH * TD];
+  for (int i = threadIdx.x; i < 256; i += kFThreads) tab256[i] = P.tabs->exp2_j256[i];
   int* const myE = &accE_s[0][threadIdx.x];
 #pragma unroll
-  for (int pq = 0; pq < TH * TD; ++pq) myE[pq * kThreads] = 0;
+  for (int pq = 0; pq < TH * TD; ++pq) myE[pq * kFThreads] = 0;
 
   int b = blockIdx.x;
   const int chunk = b % P.ksplit;  b /= P.ksplit;
@@ -372,7 +382,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
   const int bx = 1 << P.bx_log2;
   const int col = cg * bx + (threadIdx.x & (bx - 1));
   const int rsub = threadIdx.x >> P.bx_log2;
-  const int by = kThreads >> P.bx_log2;
+  const int by = kFThreads >> P.bx_log2;
   const bool valid = col < P.N;
 
   {
@@ -478,7 +488,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
               for (int j = 0; j < TD; ++j) {
                 const int hi = __double2hiint(accP[i][j]);
                 const int ex = (hi >> 20) - 1023;
-                myE[(i * TD + j) * kThreads] += ex;
+                myE[(i * TD + j) * kFThreads] += ex;
                 accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
               }
             drift = 0;
@@ -530,7 +540,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
               for (int j = 0; j < TD; ++j) {
                 const int E = max(eA[j], eb);
                 accP[i][j] *= (scale2(mA[j], eA[j] - E) + scale2(mB, eb - E));
-                myE[(i * TD + j) * kThreads] += E;
+                myE[(i * TD + j) * kFThreads] += E;
               }
             }
           }
@@ -544,7 +554,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
       for (int j = 0; j < TD; ++j) {
         const int hi = __double2hiint(accP[i][j]);
         const int ex = (hi >> 20) - 1023;
-        myE[(i * TD + j) * kThreads] += ex;
+        myE[(i * TD + j) * kFThreads] += ex;
         accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
       }
   }
@@ -556,7 +566,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
   for (int i = 0; i < TH; ++i)
 #pragma unroll
     for (int j = 0; j < TD; ++j) {
-      const double ed = (double)accEc + (double)myE[(i * TD + j) * kThreads];
+      const double ed = (double)accEc + (double)myE[(i * TD + j) * kFThreads];
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(accP[i][j])));
       const double v = warp_sum(P.T * lnz);
       if (lane == 0) red[warp][i * TD + j] = v;
@@ -568,7 +578,7 @@ __global__ void __launch_bounds__(kThreads, 2) fe_ksum_factored_kernel(const Ksu
     if (ih < P.nh && id < P.nd) {
       double tot = 0.0;
 #pragma unroll
-      for (int w = 0; w < kWarps; ++w) tot += red[w][threadIdx.x];
+      for (int w = 0; w < kFWarps; ++w) tot += red[w][threadIdx.x];
       const size_t nout = (size_t)P.nq * P.nh * P.nd;
       P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = tot;
     }
