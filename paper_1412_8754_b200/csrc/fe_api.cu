@@ -27,7 +27,7 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 struct Tile { int th, td; };
-constexpr Tile kTiles[] = {{8, 4}, {4, 4}, {2, 8}, {1, 8}};
+constexpr Tile kTiles[] = {{8, 4}, {4, 4}, {2, 8}, {1, 8}, {16, 2}, {16, 4}};
 constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 constexpr int kStageSlots = 4;
 constexpr int kSChunksMax = 128;
@@ -191,9 +191,9 @@ int stage_lists(fe_handle* h, size_t n, cudaStream_t st, double** host_out, doub
 }
 
 // Relative cost per evaluated term of each tile (measured on B200, config-4 slice).
-// kTiles order: (8,4) (4,4) (2,8) (1,8).
-constexpr double kTileCostFactored[] = {1.00, 1.33, 1.76, 2.60};
-constexpr double kTileCostDirect[]   = {1.51, 1.00, 1.12, 1.30};
+// kTiles order: (8,4) (4,4) (2,8) (1,8) (16,2) (16,4).
+constexpr double kTileCostFactored[] = {1.00, 1.72, 2.30, 3.40, 0.91, 0.73};
+constexpr double kTileCostDirect[]   = {1.51, 1.00, 1.12, 1.30, 2.00, 3.00};
 
 int choose_tile(const fe_handle* h, int nh, int nd) {
   if (h->tile > 0) return h->tile - 1;
@@ -229,7 +229,9 @@ cudaError_t launch_ksum(int tile, int nb, int form, int mode, int grid, cudaStre
     case 0: return launch_ksum_tile<8, 4>(nb, form, mode, grid, st, P);
     case 1: return launch_ksum_tile<4, 4>(nb, form, mode, grid, st, P);
     case 2: return launch_ksum_tile<2, 8>(nb, form, mode, grid, st, P);
-    default: return launch_ksum_tile<1, 8>(nb, form, mode, grid, st, P);
+    case 3: return launch_ksum_tile<1, 8>(nb, form, mode, grid, st, P);
+    case 4: return launch_ksum_tile<16, 2>(nb, form, mode, grid, st, P);
+    default: return launch_ksum_tile<16, 4>(nb, form, mode, grid, st, P);
   }
 }
 

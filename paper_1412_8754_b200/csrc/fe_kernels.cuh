@@ -52,8 +52,9 @@ struct KsumParams {
   double* partial;                     // [ksplit][nq*nh*nd]
 };
 
-// Branch-free sqrt for normal x > 0 (callers add 1e-300 to the radicand so x = 0 cannot occur): rsqrt seed (MUFU),
-// two coupled Newton steps and one residual correction; <= 1 ulp, no slow path, so independent chains interleave.
+// Branch-free sqrt for normal x > 0 (callers add 1e-300 to the radicand so x = 0 cannot occur): rsqrt seed (MUFU,
+// ~2^-22) and two coupled Newton steps (error 2^-43, then 2^-85 + rounding): <= 1.5 ulp, no slow path, so
+// independent chains interleave.  7 FP64 instructions.
 __device__ __forceinline__ double sqrt_pos(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
@@ -63,10 +64,7 @@ __device__ __forceinline__ double sqrt_pos(double x) {
   g = fma(g, r, g);
   h = fma(h, r, h);
   r = fma(-g, h, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
-  const double d = fma(-g, g, x);
-  return fma(d, h, g);
+  return fma(g, r, g);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -362,7 +360,7 @@ __host__ __device__ constexpr int htile_stride(int TH) { return 4 + 2 * TH; }
 constexpr int kFThreads = FE_FACTORED_THREADS;   // threads per block of the factored kernel
 constexpr int kFWarps = kFThreads / 32;
 template <int NB, int FORM, int TH, int TD>
-__global__ void __launch_bounds__(kFThreads, FE_FACTORED_MINBLOCKS) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
+__global__ void __launch_bounds__(kFThreads, (TH * TD > 32 ? 2 : FE_FACTORED_MINBLOCKS)) fe_ksum_factored_kernel(const KsumParams P, const FactoredConsts fc) {
   __shared__ double tab256[256];
   __shared__ double hv_s[TH], rho_s[TH], sig_s[TH], d2v_s[TD], hinfo_s[4];
   __shared__ int accE_s[TH * TD][kFThreads];        // robust-path exponent sums, [pair][thread]
@@ -497,36 +495,45 @@ __global__ void __launch_bounds__(kFThreads, FE_FACTORED_MINBLOCKS) fe_ksum_fact
 
           if (fast) {
             accEc += Eref;
-            double Ap[TD], Bp[TH];
+            constexpr int HC = TH < 8 ? TH : 8;                            // h values handled per register chunk
+            double Ap[TD], Bp[HC];
 #pragma unroll
             for (int j = 0; j < TD; ++j) Ap[j] = scale2(mA[j], eA[j] - Eref);
             if (hrec) {
               // Pm = e^{(d0-hmin)/T} (the largest e^{+y_i/T}) and Mm = C / Pm = e^{(hmax-d0)/T} (the largest
               // e^{-y_i/T}); the other h values of the tile by the host-made ratios <= 1
-              const int eb = ebB;
-              const double mb = mbB, rc = rcB;
               const bool pos = dhi >= 0.0;
-              const int pe = pos ? eb : -eb;
-              const double P0 = scale2(pos ? mb : rc, pe - Eref);                 // e^{(d0-hmin)/T} 2^-Eref
-              const double M0 = scale2((pos ? rc : mb) * mC, eC - pe - Eref);     // e^{(hmax-d0)/T} 2^-Eref
+              const int pe = pos ? ebB : -ebB;
+              const double P0 = scale2(pos ? mbB : rcB, pe - Eref);                 // e^{(d0-hmin)/T} 2^-Eref
+              const double M0 = scale2((pos ? rcB : mbB) * mC, eC - pe - Eref);     // e^{(hmax-d0)/T} 2^-Eref
 #pragma unroll
-              for (int i = 0; i < TH; ++i) Bp[i] = fma(M0, sig_s[i], P0 * rho_s[i]);
+              for (int i0 = 0; i0 < TH; i0 += HC) {
+#pragma unroll
+                for (int i = 0; i < HC; ++i) Bp[i] = fma(M0, sig_s[i0 + i], P0 * rho_s[i0 + i]);
+#pragma unroll
+                for (int i = 0; i < HC; ++i)
+#pragma unroll
+                  for (int j = 0; j < TD; ++j) accP[i0 + i][j] *= (Ap[j] + Bp[i]);
+              }
             } else {
               const bool fixB = __any_sync(wmask, eBlo < 28);
 #pragma unroll
-              for (int i = 0; i < TH; ++i) {
-                const double ad = fabs(d0 - hv_s[i]);
-                const double t = fma(ad, fc.c1, MAGIC);
-                const int eb = exp_k(t);
-                double mB = exp_mant(ad, t, fc, tab256);
-                if (fixB) mB = cosh_fix(mB, eb);
-                Bp[i] = scale2(mB, eb - Eref);
+              for (int i0 = 0; i0 < TH; i0 += HC) {
+#pragma unroll
+                for (int i = 0; i < HC; ++i) {
+                  const double ad = fabs(d0 - hv_s[i0 + i]);
+                  const double t = fma(ad, fc.c1, MAGIC);
+                  const int eb = exp_k(t);
+                  double mB = exp_mant(ad, t, fc, tab256);
+                  if (fixB) mB = cosh_fix(mB, eb);
+                  Bp[i] = scale2(mB, eb - Eref);
+                }
+#pragma unroll
+                for (int i = 0; i < HC; ++i)
+#pragma unroll
+                  for (int j = 0; j < TD; ++j) accP[i0 + i][j] *= (Ap[j] + Bp[i]);
               }
             }
-#pragma unroll
-            for (int i = 0; i < TH; ++i)
-#pragma unroll
-              for (int j = 0; j < TD; ++j) accP[i][j] *= (Ap[j] + Bp[i]);
           } else {
             const bool fixB = __any_sync(wmask, eBlo < 28);
 #pragma unroll

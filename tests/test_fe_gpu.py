@@ -85,7 +85,7 @@ def test_config2_two_band_full_parity(fe, oracle):
     assert np.array_equal(om, om_w)             # windowed evaluation is bit-identical to direct
 
 
-@pytest.mark.parametrize("tile", [1, 2, 3, 4])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("mode", [0, 1, 2])
 def test_ragged_two_band_all_tiles(fe, oracle, tile, mode):
     """Odd N (ragged column group), list lengths that divide no tile, off-grid q, negative h and Delta."""
@@ -108,7 +108,7 @@ def test_factored_kernel_every_code_path(fe, oracle, flags):
                      (W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=16, nd=32), (0.001, 0.01)),
                      (W.ragged(seed=29, N=50, nq=1, nh=9, nd=5, model=W.MODEL_ONE_BAND), (0.02,))):
         for T in temps:
-            for tile in (1, 2):
+            for tile in (1, 2, 5, 6):
                 parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED, tile=tile, flags=flags)
 
 
