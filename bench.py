@@ -44,6 +44,7 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
+    ("factored", (16, 4)): (4.20, 5.62, "ncu, profiles/r1c_ksum_factored_16x4_raw.csv"),
     ("direct", (4, 4)): (40.6, 61.3, "SASS count"),
     ("direct", (8, 4)): (39.4, 59.4, "SASS count"),
 }
