@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Omega(Delta; q, h, T) hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mode factored|direct|windowed]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mode coop|factored|direct|windowed]
 
 Workload (config.workload): BASELINE.json configs[3] "cfg4_fflo_N1024": two-band s+- model, N = 1024 x 1024 k-grid,
 32 q along (1,1), 64 h, 512 Delta -- the configuration north_star quotes its FP64-roofline target on.
@@ -147,7 +147,8 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="factored", choices=["factored", "direct", "windowed"])
+    ap.add_argument("--mode", default="coop", choices=["coop", "factored", "direct", "windowed"])
+    ap.add_argument("--shape", type=int, default=0, help="block shape of the cooperative kernel (0 = auto)")
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--q-per-step", type=int, default=0, help="q-values per step (0 = the whole q list)")
     ap.add_argument("--tile", type=int, default=0)
@@ -182,11 +183,13 @@ def main():
     else:
         q_all = w.q
     temps = list(w.T)
-    mode = {"factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT, "windowed": fe.EVAL_WINDOWED}[args.mode]
+    mode = {"coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
+            "windowed": fe.EVAL_WINDOWED}[args.mode]
 
     F = fe.FreeEnergy(w.params, w.N, temps[0])
     F.set_eval_mode(mode)
     F.set_tuning(args.tile, 0)
+    F.set_coop_shape(args.shape)
     F.enable_timing(True)
     stream = torch.cuda.current_stream()
     omega = torch.empty((nq_step, w.nh, w.nd), dtype=torch.float64, device="cuda")

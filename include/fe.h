@@ -46,8 +46,13 @@ extern "C" {
 #define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
 #define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
 
-/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all three compute the same sums ----
- * FACTORED: default.  Uses 2cosh(d/T) + 2cosh(R/T) = B(h) + A(Delta): per (k, band) TH + TD exponentials in
+/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all four compute the same sums ----
+ * COOP    : default.  The factored form below, block-cooperative: a thread block owns one (h, Delta) block tile and
+ *           a chunk of k-points; the WD + WH exponentials per (k, band) are computed once per block and shared
+ *           through shared memory; every thread keeps a TH x TD register tile of running products over all k of
+ *           the chunk (no cross-thread reduction).  Falls back to FACTORED when the grid is much smaller than a
+ *           block tile (e.g. a single h value) unless a shape is forced with fe_set_coop_shape.
+ * FACTORED: per-thread version.  Uses 2cosh(d/T) + 2cosh(R/T) = B(h) + A(Delta): per (k, band) TH + TD exponentials in
  *           extended range (fp64 mantissa + int exponent), per term one add and one multiply into a running
  *           product; the logarithm is taken once per thread at the end.
  * DIRECT  : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5
@@ -57,6 +62,7 @@ extern "C" {
 #define FE_EVAL_FACTORED 0
 #define FE_EVAL_DIRECT   1
 #define FE_EVAL_WINDOWED 2
+#define FE_EVAL_COOP     3
 
 typedef struct fe_handle fe_handle; /* opaque; owns device scratch (trig tables, partial sums, staging) */
 
@@ -81,7 +87,7 @@ int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** ou
 /* Change T (> 0, finite) for subsequent calls (config 4 scans two temperatures).  Host-only, cheap. */
 int fe_set_temperature(fe_handle* h, double T);
 
-/* Select FE_EVAL_FACTORED (default), FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
+/* Select FE_EVAL_COOP (default), FE_EVAL_FACTORED, FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
 int fe_set_eval_mode(fe_handle* h, int32_t mode);
 
 /* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,
@@ -123,8 +129,8 @@ int fe_scan_host(fe_handle* h,
 int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
 
-/* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode,
- * rows per k-chunk}.  Host-only. */
+/* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode actually
+ * used, rows per k-chunk}; for FE_EVAL_COOP: {WH, WD, ksplit, grid blocks, mode, k-points per chunk}.  Host-only. */
 int fe_get_last_launch_info(fe_handle* h, int32_t* info6);
 
 /* Number of kernel launches this handle has issued since creation (all kernels of this library). */
@@ -134,7 +140,12 @@ int fe_get_launch_count(fe_handle* h, int64_t* launches);
  * target_blocks: minimum number of thread blocks K1 should be split into (0 = auto).               */
 int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks);
 int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past the end of the table */
-/* Test hook for FE_EVAL_FACTORED: bit 0 = always take the robust per-pair path, bit 1 = never use the per-tile
+/* FE_EVAL_COOP block shape: 0 = auto, else index (from 1) into the built-in shape table; forcing a shape also
+ * disables the fallback to FE_EVAL_FACTORED.  fe_coop_shape_info: info6 = {TH, TD, WH, WD, threads per block,
+ * resident blocks per SM}; FE_EINVAL past the end of the table. */
+int fe_set_coop_shape(fe_handle* h, int32_t shape);
+int fe_coop_shape_info(int32_t shape, int32_t* info6);
+/* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP: bit 0 = always take the robust per-pair path, bit 1 = never use the per-tile
  * h recurrence.  Results are the same sums; only the code path changes (lets tests cover each path).       */
 int fe_set_debug_flags(fe_handle* h, int32_t flags);
 

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfe.so")
 SOURCES = [os.path.join(CSRC, "fe_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "fe_kernels.cuh"), os.path.join(CSRC, "fe_math.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "fe_kernels.cuh"), os.path.join(CSRC, "fe_ksum_coop.cuh"), os.path.join(CSRC, "fe_math.cuh"),
                   os.path.join(ROOT, "include", "fe.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -9,6 +9,7 @@
 
 #include "../../include/fe.h"
 #include "fe_kernels.cuh"
+#include "fe_ksum_coop.cuh"
 
 namespace {
 
@@ -29,6 +30,11 @@ int cuda_fail(cudaError_t e, const char* what) {
 struct Tile { int th, td; };
 constexpr Tile kTiles[] = {{8, 4}, {4, 4}, {2, 8}, {1, 8}, {16, 2}, {16, 4}};
 constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
+// Shapes of the block-cooperative kernel K1c: register tile TH x TD per thread, LH lanes of a warp along h, NW warps,
+// KB k-points per shared-memory sub-batch, MINB resident blocks per SM.  Block tile = (TH LH) x (TD NW 32/LH).
+struct CoopShape { int th, td, lh, nw, kb, minb; };
+constexpr CoopShape kCoopShapes[] = {{16, 4, 4, 4, 4, 2}, {16, 4, 1, 4, 2, 2}, {8, 4, 4, 4, 4, 3}, {8, 4, 1, 4, 2, 2}};
+constexpr int kNumCoopShapes = sizeof(kCoopShapes) / sizeof(kCoopShapes[0]);
 constexpr int kStageSlots = 4;
 constexpr int kSChunksMax = 128;
 
@@ -46,10 +52,11 @@ struct fe_handle {
   fe_model_params p;
   int32_t N = 0;
   double T = 0;
-  int32_t mode = FE_EVAL_FACTORED;
+  int32_t mode = FE_EVAL_COOP;
   int32_t tile = 0;            // 0 = auto, else 1 + index
   int32_t target_blocks = 0;   // 0 = auto
   int32_t debug_flags = 0;
+  int32_t coop_shape = 0;      // 0 = auto, else 1 + index into kCoopShapes
   int device = 0;
   int sm_count = 148;
   int nb = 1;
@@ -195,9 +202,12 @@ int stage_lists(fe_handle* h, size_t n, cudaStream_t st, double** host_out, doub
 constexpr double kTileCostFactored[] = {1.00, 1.72, 2.30, 3.40, 0.91, 0.73};
 constexpr double kTileCostDirect[]   = {1.51, 1.00, 1.12, 1.30, 2.00, 3.00};
 
-int choose_tile(const fe_handle* h, int nh, int nd) {
-  if (h->tile > 0) return h->tile - 1;
-  const double* cost_tab = h->mode == FE_EVAL_FACTORED ? kTileCostFactored : kTileCostDirect;
+// cost of one K1c pair relative to kTileCostFactored's unit (measured, config-4 step)
+constexpr double kCoopVsFactored = 0.28;
+
+int choose_tile_mode(int forced_tile, int mode, int nh, int nd) {
+  if (forced_tile > 0) return forced_tile - 1;
+  const double* cost_tab = mode == FE_EVAL_FACTORED ? kTileCostFactored : kTileCostDirect;
   int best = 0; double best_cost = 1e300;
   for (int t = 0; t < kNumTiles; ++t) {
     const double padded = (double)((nh + kTiles[t].th - 1) / kTiles[t].th * kTiles[t].th) *
@@ -207,6 +217,7 @@ int choose_tile(const fe_handle* h, int nh, int nd) {
   }
   return best;
 }
+
 
 template <int NB, int FORM, int TH, int TD>
 cudaError_t launch_ksum_mode(int mode, int grid, cudaStream_t st, const KsumParams& P) {
@@ -235,6 +246,60 @@ cudaError_t launch_ksum(int tile, int nb, int form, int mode, int grid, cudaStre
   }
 }
 
+
+// ---- K1c (block-cooperative factored kernel) -------------------------------------------------------
+template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
+cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
+  using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
+  auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB>;
+  static bool attr_set = false;     // per instantiation; the attribute is sticky for the function
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  kern<<<grid, G::NT, G::smem_bytes, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int TH, int TD, int LH, int NW, int KB, int MINB>
+cudaError_t launch_coop_shape(int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
+  if (nb == 1) return form == 0 ? launch_coop_inst<1, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
+                                : launch_coop_inst<1, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
+  return form == 0 ? launch_coop_inst<2, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
+                   : launch_coop_inst<2, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
+}
+
+cudaError_t launch_coop(int shape, int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
+  switch (shape) {
+    case 0: return launch_coop_shape<16, 4, 4, 4, 4, 2>(nb, form, grid, st, P);
+    case 1: return launch_coop_shape<16, 4, 1, 4, 2, 2>(nb, form, grid, st, P);
+    case 2: return launch_coop_shape<8, 4, 4, 4, 4, 3>(nb, form, grid, st, P);
+    default: return launch_coop_shape<8, 4, 1, 4, 2, 2>(nb, form, grid, st, P);
+  }
+}
+
+// Relative cost per evaluated pair of each coop shape: pair work 2 TH TD per slot and thread plus the thread's share
+// of the (WD + WH) exponentials (~20 FP64 instructions each).
+double coop_shape_cost(const CoopShape& s) {
+  const int nt = s.nw * 32, wh = s.th * s.lh, wd = s.td * s.nw * (32 / s.lh);
+  const double pair = 2.0 * s.th * s.td, expo = 20.0 * (wh + wd) / nt;
+  return (pair + expo) / pair * (s.th * s.td >= 64 ? 1.0 : 1.08);
+}
+
+int choose_coop_shape(const fe_handle* h, int nh, int nd) {
+  if (h->coop_shape > 0) return h->coop_shape - 1;
+  int best = 0; double best_cost = 1e300;
+  for (int t = 0; t < kNumCoopShapes; ++t) {
+    const CoopShape& s = kCoopShapes[t];
+    const int wh = s.th * s.lh, wd = s.td * s.nw * (32 / s.lh);
+    const double padded = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd);
+    const double cost = padded * coop_shape_cost(s);
+    if (cost < best_cost * (1.0 - 1e-12)) { best_cost = cost; best = t; }
+  }
+  return best;
+}
+
 int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh, const double* delta, int32_t nd) {
   if (!q_xy || !h_list || !delta) { snprintf(g_errbuf, sizeof g_errbuf, "a list pointer is NULL"); return FE_EINVAL; }
   if (nq < 1 || nh < 1 || nd < 1) { snprintf(g_errbuf, sizeof g_errbuf, "nq, nh, nd must be >= 1"); return FE_EINVAL; }
@@ -248,8 +313,25 @@ int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh
 int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                     const double* delta, int32_t nd, double* omega_dev, cudaStream_t st) {
   const int N = h->N;
+  // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
+  int mode = h->mode;
+  int cshape = 0;
+  if (mode == FE_EVAL_COOP) {
+    cshape = choose_coop_shape(h, nh, nd);
+    if (h->coop_shape == 0) {
+      const CoopShape& cs = kCoopShapes[cshape];
+      const int wh = cs.th * cs.lh, wd = cs.td * cs.nw * (32 / cs.lh);
+      const double coop_cost = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd) *
+                               coop_shape_cost(cs) * kCoopVsFactored;
+      const int lt = choose_tile_mode(0, FE_EVAL_FACTORED, nh, nd);
+      const double legacy_cost = (double)((nh + kTiles[lt].th - 1) / kTiles[lt].th * kTiles[lt].th) *
+                                 (double)((nd + kTiles[lt].td - 1) / kTiles[lt].td * kTiles[lt].td) * kTileCostFactored[lt];
+      if (legacy_cost < coop_cost) mode = FE_EVAL_FACTORED;
+    }
+  }
+  const bool coop = mode == FE_EVAL_COOP;
   // ---- stage lists: [q (2nq) | h (nh) | delta^2 (nd)] ----
-  const int tile = choose_tile(h, nh, nd);
+  const int tile = choose_tile_mode(mode == h->mode ? h->tile : 0, mode, nh, nd);
   const int TH = kTiles[tile].th, TD = kTiles[tile].td;
   const int ntile_h = (nh + TH - 1) / TH;
   const int hstride = htile_stride(TH);
@@ -298,7 +380,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   P.debug_flags = h->debug_flags;
   P.ntile_h = (nh + TH - 1) / TH;
   P.ntile_d = (nd + TD - 1) / TD;
-  const int bthreads = h->mode == FE_EVAL_FACTORED ? kFThreads : kThreads;
+  const int bthreads = mode == FE_EVAL_FACTORED ? kFThreads : kThreads;
   int bxl = 0;
   while ((1 << bxl) < bthreads) ++bxl;           // all threads along kx when N allows it
   while (bxl > 5 && (1 << (bxl - 1)) >= N) --bxl;
@@ -313,6 +395,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   if (nrs < 1) nrs = 1;
   int rpc = (int)((N + nrs - 1) / nrs);
   rpc = (rpc + by - 1) / by * by;                // whole row-lane strides per chunk
+  double coop_max_k = 1e18;                      // k-points per chunk K1c may sum into its int32 exponent sums
   {
     // Range guards of the factored kernel: binary exponents x/(T ln2) are summed in int32 per thread, and the
     // range reduction needs x/T * 64/ln2 < 2^37.  |E_k| <= W, so R <= W + |mu| + |Delta eta|, |d| <= W + |h|.
@@ -329,6 +412,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     }
     const double ebound = xmax / 0.6931471805599453 + 4.0;            // max binary exponent of one term
     const double max_terms = 2.0e9 / ebound;                          // per thread and accumulator
+    coop_max_k = floor(max_terms / h->nb);
     int max_rows = (int)fmin((double)N, floor(max_terms / h->nb)) * by;
     if (max_rows < by) max_rows = by;
     if (rpc > max_rows) rpc = max_rows / by * by;
@@ -336,7 +420,46 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   P.rows_per_chunk = rpc;
   P.nrs = (N + rpc - 1) / rpc;
   P.ksplit = P.ncg * P.nrs;
-  const long long grid_ll = ntiles * P.ksplit;
+  long long grid_ll = ntiles * P.ksplit;
+
+  // ---- K1c geometry: block tiles x k-chunks; the grid is sized to whole waves of resident blocks ----
+  CoopParams CP;
+  if (coop) {
+    const CoopShape& cs = kCoopShapes[cshape];
+    const int nt = cs.nw * 32, wh = cs.th * cs.lh, wd = cs.td * cs.nw * (32 / cs.lh);
+    CP.mc = P.mc; CP.fc = make_factored(h->T); CP.T = h->T;
+    CP.N = N; CP.nq = nq; CP.nh = nh; CP.nd = nd;
+    CP.ntile_h = (nh + wh - 1) / wh; CP.ntile_d = (nd + wd - 1) / wd;
+    CP.debug_flags = h->debug_flags;
+    CP.nk = (unsigned long long)N * (unsigned long long)N;
+    const long long ctiles = (long long)nq * CP.ntile_h * CP.ntile_d;
+    const long long wave = (long long)h->sm_count * cs.minb;
+    const long long max_split = (long long)((CP.nk + nt - 1) / nt);          // at least one thread-batch per chunk
+    long long min_split = (long long)ceil((double)CP.nk / fmax(1.0, floor(coop_max_k / nt) * nt));
+    if (min_split < 1) min_split = 1;
+    long long ks;
+    if (h->target_blocks > 0) {
+      ks = (h->target_blocks + ctiles - 1) / ctiles;
+    } else {
+      // >= 8 waves; among the next candidates take the split whose last wave is fullest
+      const long long ks0 = (8 * wave + ctiles - 1) / ctiles;
+      ks = ks0; double best_eff = 0;
+      for (long long c = ks0; c <= 2 * ks0 + 1; ++c) {
+        const long long g = ctiles * c, waves = (g + wave - 1) / wave;
+        const double eff = (double)g / (double)(waves * wave);
+        if (eff > best_eff + 1e-9) { best_eff = eff; ks = c; }
+      }
+    }
+    if (ks < min_split) ks = min_split;
+    if (ks > max_split) ks = max_split;
+    if (ks < 1) ks = 1;
+    unsigned long long kc = (CP.nk + ks - 1) / ks;
+    kc = (kc + nt - 1) / nt * nt;
+    CP.kc = kc;
+    CP.ksplit = (int32_t)((CP.nk + kc - 1) / kc);
+    P.ksplit = CP.ksplit;
+    grid_ll = ctiles * CP.ksplit;
+  }
   if (grid_ll > 2147483647LL) { snprintf(g_errbuf, sizeof g_errbuf, "grid too large"); return FE_EINVAL; }
 
   const size_t nout = (size_t)nq * nh * nd;
@@ -366,9 +489,17 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     h->launches++;
   }
   h->last_info[0] = TH; h->last_info[1] = TD; h->last_info[2] = P.ksplit; h->last_info[3] = (int32_t)grid_ll;
-  h->last_info[4] = h->mode; h->last_info[5] = P.rows_per_chunk;
+  h->last_info[4] = mode; h->last_info[5] = P.rows_per_chunk;
+  if (coop) {
+    const CoopShape& cs = kCoopShapes[cshape];
+    h->last_info[0] = cs.th * cs.lh; h->last_info[1] = cs.td * cs.nw * (32 / cs.lh);     // block tile WH x WD
+    h->last_info[5] = (int32_t)(CP.kc < 2147483647ULL ? CP.kc : 2147483647ULL);          // k-points per chunk
+    CP.coltab = h->d_coltab; CP.rowtab = h->d_rowtab; CP.h = d_h; CP.d2 = d_d2; CP.tabs = h->d_tabs;
+    CP.partial = h->d_partial;
+  }
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
-  FE_CUDA(launch_ksum(tile, h->nb, h->p.form_factor, h->mode, (int)grid_ll, st, P));
+  if (coop) FE_CUDA(launch_coop(cshape, h->nb, h->p.form_factor, (int)grid_ll, st, CP));
+  else      FE_CUDA(launch_ksum(tile, h->nb, h->p.form_factor, mode, (int)grid_ll, st, P));
   h->launches++;
   if (h->timing) {
     FE_CUDA(cudaEventRecord(h->ev1, st));
@@ -448,7 +579,7 @@ int fe_set_temperature(fe_handle* h, double T) {
 
 int fe_set_eval_mode(fe_handle* h, int32_t mode) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
-  if (mode != FE_EVAL_FACTORED && mode != FE_EVAL_DIRECT && mode != FE_EVAL_WINDOWED) {
+  if (mode != FE_EVAL_FACTORED && mode != FE_EVAL_DIRECT && mode != FE_EVAL_WINDOWED && mode != FE_EVAL_COOP) {
     snprintf(g_errbuf, sizeof g_errbuf, "unknown eval mode %d", mode); return FE_EINVAL; }
   h->mode = mode;
   return FE_OK;
@@ -459,6 +590,22 @@ int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks) {
   if (tile < 0 || tile > kNumTiles || target_blocks < 0) {
     snprintf(g_errbuf, sizeof g_errbuf, "tile must be in [0, %d], target_blocks >= 0", kNumTiles); return FE_EINVAL; }
   h->tile = tile; h->target_blocks = target_blocks;
+  return FE_OK;
+}
+
+int fe_set_coop_shape(fe_handle* h, int32_t shape) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (shape < 0 || shape > kNumCoopShapes) {
+    snprintf(g_errbuf, sizeof g_errbuf, "shape must be in [0, %d]", kNumCoopShapes); return FE_EINVAL; }
+  h->coop_shape = shape;
+  return FE_OK;
+}
+
+int fe_coop_shape_info(int32_t shape, int32_t* info6) {
+  if (shape < 1 || shape > kNumCoopShapes || !info6) { snprintf(g_errbuf, sizeof g_errbuf, "no such shape"); return FE_EINVAL; }
+  const CoopShape& s = kCoopShapes[shape - 1];
+  info6[0] = s.th; info6[1] = s.td; info6[2] = s.th * s.lh; info6[3] = s.td * s.nw * (32 / s.lh);
+  info6[4] = s.nw * 32; info6[5] = s.minb;
   return FE_OK;
 }
 

@@ -14,10 +14,10 @@ import numpy as np
 from . import build as _build
 
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
-EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED = 0, 1, 2
+EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP = 0, 1, 2, 3
 
 EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_scan_host",
-           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags",
+           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
 
@@ -67,6 +67,8 @@ def lib():
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
     L.fe_set_debug_flags.argtypes = [vp, C.c_int32]
+    L.fe_set_coop_shape.argtypes = [vp, C.c_int32]
+    L.fe_coop_shape_info.argtypes = [C.c_int32, ip]
     L.fe_fp64_peak_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_float), dp, vp]
     L.fe_debug_math.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp]
     L.fe_destroy.argtypes = [vp]
@@ -119,6 +121,16 @@ def tiles():
     return out
 
 
+def coop_shapes():
+    """[(TH, TD, WH, WD, threads, blocks_per_sm), ...] of the FE_EVAL_COOP shape table (index + 1 = shape id)."""
+    out, i = [], 1
+    a = (C.c_int32 * 6)()
+    while lib().fe_coop_shape_info(i, a) == FE_OK:
+        out.append(tuple(a))
+        i += 1
+    return out
+
+
 def fp64_peak_probe(blocks=148 * 16, iters=1 << 16, stream=None):
     """Measured DFMA rate of the current device: returns (dfma_per_second, ms)."""
     ms, cnt = C.c_float(), C.c_double()
@@ -158,6 +170,9 @@ class FreeEnergy:
 
     def set_tuning(self, tile=0, target_blocks=0):
         _check(lib().fe_set_tuning(self._h, int(tile), int(target_blocks)))
+
+    def set_coop_shape(self, shape=0):
+        _check(lib().fe_set_coop_shape(self._h, int(shape)))
 
     def set_debug_flags(self, flags):
         _check(lib().fe_set_debug_flags(self._h, int(flags)))

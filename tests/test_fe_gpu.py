@@ -20,11 +20,15 @@ GAP = 1e-10
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
-def run_gpu(fe, w, T, mode=0, tile=0, target_blocks=0, flags=0):
+def run_gpu(fe, w, T, mode=None, tile=0, target_blocks=0, flags=0, shape=0):
+    """mode None = the library default (FE_EVAL_COOP, falling back to FACTORED on tiny grids); shape > 0 forces a
+    block shape of the cooperative kernel (and with it the cooperative kernel itself)."""
     import torch
     with fe.FreeEnergy(w.params, w.N, T) as F:
-        F.set_eval_mode(mode)
+        if mode is not None:
+            F.set_eval_mode(mode)
         F.set_tuning(tile, target_blocks)
+        F.set_coop_shape(shape)
         F.set_debug_flags(flags)
         om = F.omega_grid(w.q, w.h, w.delta)
         idx, ds, os_ = F.argmin(om, w.delta)
@@ -72,13 +76,18 @@ def parity(fe, oracle, w, T, **kw):
 # --------------------------------------------------------------------------------------------------
 def test_config1_bcs_full_parity(fe, oracle):
     w = W.config(1)
-    for mode in (0, 1, 2):
+    for mode in (0, 1, 2, 3):
         om, ref = parity(fe, oracle, w, w.T[0], mode=mode)
+    for shape in range(1, len(fe.coop_shapes()) + 1):
+        parity(fe, oracle, w, w.T[0], mode=fe.EVAL_COOP, shape=shape)
     assert int(np.argmin(om[0, 0])) == 47
 
 
 def test_config2_two_band_full_parity(fe, oracle):
     w = W.config(2)
+    parity(fe, oracle, w, w.T[0])
+    for shape in range(1, len(fe.coop_shapes()) + 1):
+        parity(fe, oracle, w, w.T[0], mode=fe.EVAL_COOP, shape=shape)
     parity(fe, oracle, w, w.T[0], mode=fe.EVAL_FACTORED)
     om, ref = parity(fe, oracle, w, w.T[0], mode=fe.EVAL_DIRECT)
     om_w, _ = parity(fe, oracle, w, w.T[0], mode=fe.EVAL_WINDOWED)
@@ -91,6 +100,17 @@ def test_ragged_two_band_all_tiles(fe, oracle, tile, mode):
     """Odd N (ragged column group), list lengths that divide no tile, off-grid q, negative h and Delta."""
     w = W.ragged(seed=7, N=45, nq=3, nh=5, nd=37)
     parity(fe, oracle, w, w.T[0], tile=tile, mode=mode)
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("shape", [1, 2, 3, 4])
+def test_ragged_two_band_all_coop_shapes(fe, oracle, shape, flags):
+    """The block-cooperative kernel on grids that divide no block tile (padding in h, Delta and the k-chunk tail),
+    fast slots (flags 0) and every slot forced through the robust per-pair path (flags 1)."""
+    w = W.ragged(seed=7, N=45, nq=3, nh=5, nd=37)
+    parity(fe, oracle, w, w.T[0], mode=fe.EVAL_COOP, shape=shape, flags=flags)
+    w = W.ragged(seed=8, N=61, nq=2, nh=70, nd=150)          # more than one block tile in h and in Delta
+    parity(fe, oracle, w, w.T[0], mode=fe.EVAL_COOP, shape=shape, flags=flags)
 
 
 @pytest.mark.parametrize("tile", [0, 1, 4])
@@ -112,6 +132,16 @@ def test_factored_kernel_every_code_path(fe, oracle, flags):
                 parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED, tile=tile, flags=flags)
 
 
+@pytest.mark.parametrize("flags", [0, 1])
+def test_coop_kernel_every_code_path(fe, oracle, flags):
+    for w, temps in ((W.ragged(seed=23, N=70, nq=2, nh=11, nd=9), (0.004, 0.05, 1e-4)),
+                     (W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=16, nd=32), (0.001, 0.01)),
+                     (W.ragged(seed=29, N=50, nq=1, nh=9, nd=5, model=W.MODEL_ONE_BAND), (0.02,))):
+        for T in temps:
+            for shape in (1, 2, 3, 4):
+                parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=shape, flags=flags)
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
@@ -121,13 +151,17 @@ def test_factored_extreme_spreads(fe, oracle):
     w = W.Workload("wide_h", p, 40, (0.001,), np.array([[0.3, 0.1], [0.0, 0.0]]), h, d)
     for T in (0.001, 2e-4, 3e-5, 0.2):
         parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED)
+        for shape in (1, 2):      # the block tile spans the whole wide h list: robust slots chosen on their own
+            parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=shape)
 
 
 def test_ksplit_variants_agree_and_match(fe, oracle):
     """Different k-chunkings (row splits) change only the summation tree: all within 1e-12 of the oracle."""
     w = W.ragged(seed=3, N=300, nq=2, nh=4, nd=8)
     for tb in (1, 64, 5000, 100000):
-        parity(fe, oracle, w, w.T[0], target_blocks=tb)
+        parity(fe, oracle, w, w.T[0], target_blocks=tb, mode=fe.EVAL_FACTORED)
+        parity(fe, oracle, w, w.T[0], target_blocks=tb, mode=fe.EVAL_COOP, shape=1)
+        parity(fe, oracle, w, w.T[0], target_blocks=tb, mode=fe.EVAL_COOP, shape=4)
 
 
 def test_interior_minimum_grids(fe, oracle):
@@ -136,6 +170,7 @@ def test_interior_minimum_grids(fe, oracle):
     for U, T in ((4.0, 0.001), (5.0, 0.01), (6.0, 0.001)):
         w = W.interior_minimum(N=64, U=U, T=T, nq=4, nh=8, nd=128)
         parity(fe, oracle, w, T, mode=fe.EVAL_WINDOWED)
+        parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=1)
         om, ref = parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED)
         am = np.argmin(ref, axis=-1)
         n_interior += int(np.sum((am > 0) & (am < w.nd - 1)))
@@ -174,6 +209,8 @@ def test_low_and_high_temperature(fe, oracle):
     for T in (1e-5, 5e-4, 0.05, 1.0, 25.0):
         for mode in (0, 1, 2):
             parity(fe, oracle, w, T, mode=mode)
+        parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=1)
+        parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=3)
 
 
 def test_determinism_bitwise(fe):
@@ -182,6 +219,12 @@ def test_determinism_bitwise(fe):
     b = run_gpu(fe, w, 0.001)
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+    for shape in (1, 3):
+        e = run_gpu(fe, w, 0.001, mode=fe.EVAL_COOP, shape=shape)
+        f = run_gpu(fe, w, 0.001, mode=fe.EVAL_COOP, shape=shape)
+        for x, y in zip(e, f):
+            assert np.array_equal(x, y)
+        assert max_rel(a[0], e[0]) < 1e-13
     c = run_gpu(fe, w, 0.001, mode=fe.EVAL_DIRECT)
     d = run_gpu(fe, w, 0.001, mode=fe.EVAL_WINDOWED)
     assert np.array_equal(c[0], d[0])
@@ -261,8 +304,9 @@ def load_golden(cfg):
     return json.load(open(path))
 
 
+@pytest.mark.parametrize("mode", [3, 0])
 @pytest.mark.parametrize("cfg", [3, 4, 5])
-def test_full_size_configs_sampled_parity(fe, cfg):
+def test_full_size_configs_sampled_parity(fe, cfg, mode):
     import torch
     g = load_golden(cfg)
     w = W.config(cfg)
@@ -272,7 +316,7 @@ def test_full_size_configs_sampled_parity(fe, cfg):
         cols = run["columns"]
         iqs = sorted(set(c["iq"] for c in cols))
         with fe.FreeEnergy(w.params, w.N, T) as F:
-            F.set_eval_mode(fe.EVAL_FACTORED)
+            F.set_eval_mode(mode)
             for iq in iqs:
                 # the launch configuration bench.py times: one q, the full (h, Delta) grid of the config
                 om = F.omega_grid(w.q[iq:iq + 1], w.h, w.delta)
