@@ -10,9 +10,10 @@
 //
 //   P0  (once per NT k-points, one k per thread)  dispersion A.1-A.4 at k and k-q, s, d0, eta^2 per band, and the
 //       block tile's exponent bounds -> a 32-byte header per (k, band) "slot": {s^2, eta^2, d0, Eref, flags}.
-//   P1  (per sub-batch of KB k-points)  the SLOTS x (WD + WH) exponentials A_j, B_i, one item per thread at a time,
-//       scaled by 2^-Eref and stored as plain doubles:  WD + WH exponentials per slot for the whole block
-//       instead of (TD + TH) per thread.
+//   P1  (per sub-batch of KB k-points)  the SLOTS x (WD + WH) exponentials A_j, B_i: a thread keeps a fixed Delta_j
+//       (and a fixed h_i) and walks the slots, four independent sqrt / exp chains at a time; results are scaled by
+//       2^-Eref and stored as plain doubles: WD + WH exponentials per slot for the whole block instead of
+//       (TD + TH) per thread.  Written into one of two buffers while P2 reads the other (one barrier per sub-batch).
 //   P2  every thread owns a fixed TH x TD register tile of the block tile for ALL k of the chunk and does, per slot,
 //       TD + TH shared-memory loads (LDS.128, mostly broadcast) and TH*TD x { DADD, DMUL }:
 //           accP_ij *= (A'_j + B'_i)                       running product, exponent taken out via Eref
@@ -27,6 +28,8 @@
 // Robust slots (wider spread, e.g. an h list spanning thousands of T): mantissa and exponent are stored
 // separately and each pair uses its own E = max(eA_j, eB_i), summed per pair in shared memory.
 #pragma once
+#include <type_traits>
+
 #include "fe_kernels.cuh"
 
 namespace fe {
@@ -62,74 +65,32 @@ struct CoopGeom {
   static constexpr int NTD = NW * LD;          // threads along Delta
   static constexpr int WH = TH * LH;           // block tile, h
   static constexpr int WD = TD * NTD;          // block tile, Delta
-  static constexpr int W = WD + WH;            // exponentials per slot
+  static constexpr int PADB = LH > 1 ? 2 : 0;  // B rows of the LH thread rows are 2 doubles apart in banks
+  static constexpr int W = WD + LH * (TH + PADB);            // doubles per slot row
   static constexpr int SLOTS = KB * NB;        // slots per sub-batch
   static constexpr int BUF_DOUBLES = SLOTS * W + SLOTS;      // values + one int2 {eref, flags} per slot
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * NT * NB + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
       sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8);
+  // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
+  // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
+  __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * (2 * NTD) + (jg / TD) * 2 + (jg & 1); }
+  __host__ __device__ static constexpr int posB(int ib) { return WD + ib + (ib / TH) * PADB; }
 };
 
-// P1 for one kind of item (A_j: KIND 0, B_i: KIND 1) of one sub-batch: U independent chains per thread so that the
-// sqrt / exp dependency chains of different items interleave in the FP64 pipe.
-template <int KIND, int SLOTS, int WD, int WH, int NT, int U>
-__device__ __forceinline__ void coop_p1(const CoopHdr* __restrict__ hdr_b, const double* __restrict__ list_s,
-                                        const double* __restrict__ tab256, const FactoredConsts& fc,
-                                        double* __restrict__ val, int* __restrict__ ev, int tid) {
-  constexpr int W = WD + WH, CNT = KIND == 0 ? WD : WH, OFF = KIND == 0 ? 0 : WD;
-  const double MAGIC = 6755399441055744.0;
-  for (int it0 = tid; it0 < SLOTS * CNT; it0 += U * NT) {
-    double x[U], m[U];
-    int e[U], eref[U], flags[U], pos[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int it = it0 + u * NT;
-      const bool act = it < SLOTS * CNT;
-      const int itc = act ? it : it0;
-      const int sl = itc / CNT, idx = itc - sl * CNT;
-      const CoopHdr hd = hdr_b[sl];
-      pos[u] = sl * W + OFF + idx;
-      eref[u] = hd.eref;
-      flags[u] = act ? hd.flags : kCoopSkip;
-      if (KIND == 0) x[u] = fma(list_s[idx], hd.g2, hd.s2);       // Eq. 4 radicand                (S5)
-      else           x[u] = fabs(hd.d0 - list_s[idx]);            // |d_i| = |d0 - h_i|
-    }
-    if (KIND == 0) {
-#pragma unroll
-      for (int u = 0; u < U; ++u) x[u] = sqrt_pos(x[u]);           // R_j
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const double t = fma(x[u], fc.c1, MAGIC);
-      e[u] = exp_k(t);
-      m[u] = exp_mant(x[u], t, fc, tab256);                        // e^{x/T} = m 2^e
-    }
-    if (KIND == 1) {
-#pragma unroll
-      for (int u = 0; u < U; ++u) m[u] = cosh_fix(m[u], e[u]);     // + e^{-x/T}: |d|/T is small on whole FFLO lines
-    } else {
-      bool any = false;
-#pragma unroll
-      for (int u = 0; u < U; ++u) any |= e[u] < 28;
-      if (any) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) m[u] = cosh_fix(m[u], e[u]);
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      if (flags[u] & kCoopSkip) continue;
-      if (flags[u] & kCoopRobust) { val[pos[u]] = m[u]; ev[pos[u]] = e[u]; }
-      else                        val[pos[u]] = scale2(m[u], e[u] - eref[u]);
-    }
-  }
+// m 2^(e - eref) for m in [0.997, 2.51); shifts below -1000 are clamped there (the value is then < 2^-500 of its
+// partner in every pair of a fast slot, so what it is exactly does not matter)
+__device__ __forceinline__ double coop_scale(double m, int shift) {
+  return __hiloint2double(__double2hiint(m) + (max(shift, -1000) << 20), __double2loint(m));
 }
 
 template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopParams P) {
   using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
   constexpr int NT = G::NT, WH = G::WH, WD = G::WD, W = G::W, SLOTS = G::SLOTS, BPS = NT / KB;
-  static_assert(NT % KB == 0 && TD % 2 == 0 && TH % 2 == 0 && W % 2 == 0 && G::BUF_DOUBLES % 2 == 0, "geometry");
+  constexpr int U = 4;                         // independent chains per thread in P1
+  static_assert(NT % KB == 0 && TD % 2 == 0 && TH % 4 == 0 && W % 2 == 0 && G::BUF_DOUBLES % 2 == 0, "geometry");
+  static_assert(WD % NT == 0 && NT % WH == 0, "P1 mapping");
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   CoopHdr* const hdr_s = reinterpret_cast<CoopHdr*>(smem_raw);                       // [NT*NB]
@@ -191,7 +152,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   const bool force_robust = (P.debug_flags & 1) != 0;
 
   // ---------------- P0: one k-point per thread -> NB slot headers (for NT consecutive k-points) ----------------
-  auto p0 = [&](int superbatch) {
+  // returns (to every thread, through the barrier) whether any of the NT*NB slots needs the robust path
+  auto p0 = [&](int superbatch) -> bool {
     const unsigned long long kidx = kbeg + (unsigned long long)superbatch * NT + tid;
     const bool valid = kidx < kend;
     const unsigned long long kk = valid ? kidx : kbeg;
@@ -204,6 +166,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     double g2 = P.mc.eta_scale;                              // eta(k)                     (S4)
     if (FORM == 1) g2 *= ct.x * rr.x;
     g2 *= g2;
+    bool any_robust = false;
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
       CoopHdr hd;
@@ -226,98 +189,185 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       hd.eref = hi - (spread >> 1);
       int flags = robust ? (kCoopRobust | (3 << 8)) : (((spread >> 1) + 4) << 8);
       if (!valid || !((P.mc.band_mask >> e) & 1)) flags = kCoopSkip;
+      any_robust |= (flags & kCoopRobust) != 0;
       hd.flags = flags;
       hdr_s[tid * NB + e] = hd;
     }
+    return __syncthreads_or(any_robust) != 0;
   };
 
   // ---------------- P1: the SLOTS x (WD + WH) exponentials of sub-batch `bt` into buffer bt & 1 ----------------
-  auto p1 = [&](int bt) {
+  // A thread keeps its Delta_j^2 (WD/NT of them) and its h_i and walks the slots, U independent chains at a time.
+  // ROB: some slot of this group of NT k-points is robust -> per-slot flag test, robust slots store (m, e).
+  auto p1 = [&](int bt, auto rob_tag) {
+    constexpr bool ROB = decltype(rob_tag)::value;
     const CoopHdr* const hdr_b = hdr_s + (bt % BPS) * SLOTS;
     double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
     int* const ev = ev_s + (bt & 1) * SLOTS * W;
     if (tid < SLOTS) reinterpret_cast<int2*>(val + SLOTS * W)[tid] = make_int2(hdr_b[tid].eref, hdr_b[tid].flags);
-    coop_p1<0, SLOTS, WD, WH, NT, 4>(hdr_b, d2_s, tab256, fc, val, ev, tid);
-    coop_p1<1, SLOTS, WD, WH, NT, 4>(hdr_b, h_s, tab256, fc, val, ev, tid);
+    auto put = [&](int pos, double m, int e, int eref, int flags) {
+      if (ROB && (flags & kCoopRobust)) { val[pos] = m; ev[pos] = e; }
+      else                              val[pos] = coop_scale(m, e - eref);
+    };
+    // ---- A_j = 2cosh(R_j/T) ----
+#pragma unroll 1
+    for (int r = 0; r < WD / NT; ++r) {
+      const int jg = tid + r * NT;
+      const double d2 = d2_s[jg];
+      const int pos = G::posA(jg);
+#pragma unroll 1
+      for (int sl0 = 0; sl0 < SLOTS; sl0 += U) {
+        double x[U], m[U];
+        int e[U], eref[U], flags[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int sl = min(sl0 + u, SLOTS - 1);
+          const double2 sg = *reinterpret_cast<const double2*>(&hdr_b[sl].s2);
+          const int2 ef = *reinterpret_cast<const int2*>(&hdr_b[sl].eref);
+          eref[u] = ef.x; flags[u] = ef.y;
+          x[u] = sqrt_pos(fma(d2, sg.y, sg.x));                      // R_j, Eq. 4 radicand           (S5)
+        }
+        bool fix = false;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const double t = fma(x[u], fc.c1, MAGIC);
+          e[u] = exp_k(t);
+          m[u] = exp_mant(x[u], t, fc, tab256);                      // e^{R/T} = m 2^e
+          fix |= e[u] < 28;
+        }
+        if (fix) {
+#pragma unroll
+          for (int u = 0; u < U; ++u) m[u] = cosh_fix(m[u], e[u]);   // + e^{-R/T}
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+          if (sl0 + u < SLOTS) put((sl0 + u) * W + pos, m[u], e[u], eref[u], flags[u]);
+      }
+    }
+    // ---- B_i = 2cosh((d0 - h_i)/T): NT / WH slots per pass ----
+    {
+      constexpr int SPP = NT / WH, PASSES = (SLOTS + SPP - 1) / SPP;
+      const int ib = tid % WH, slb = tid / WH;
+      const double hv = h_s[ib];
+      const int pos = G::posB(ib);
+#pragma unroll 1
+      for (int p0i = 0; p0i < PASSES; p0i += U) {
+        double x[U], m[U];
+        int e[U], eref[U], flags[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int sl = min(slb + (p0i + u) * SPP, SLOTS - 1);
+          const double d0 = hdr_b[sl].d0;
+          const int2 ef = *reinterpret_cast<const int2*>(&hdr_b[sl].eref);
+          eref[u] = ef.x; flags[u] = ef.y;
+          x[u] = fabs(d0 - hv);                                      // |d_i| = |d0 - h_i|
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const double t = fma(x[u], fc.c1, MAGIC);
+          e[u] = exp_k(t);
+          m[u] = cosh_fix(exp_mant(x[u], t, fc, tab256), e[u]);      // |d|/T is small on whole lines of the zone
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int sl = slb + (p0i + u) * SPP;
+          if (sl < SLOTS) put(sl * W + pos, m[u], e[u], eref[u], flags[u]);
+        }
+      }
+    }
   };
 
-  p0(0);
-  __syncthreads();
-  p1(0);
+  bool sb_robust = p0(0);
+  if (sb_robust) p1(0, std::true_type{}); else p1(0, std::false_type{});
   __syncthreads();
 
+  constexpr int HC = TH / 2;                     // the h half-tile handled between two shared-memory fetches
 #pragma unroll 1
   for (int bt = 0; bt < nbatch; ++bt) {
     if (bt + 1 < nbatch) {
-      if ((bt + 1) % BPS == 0) {        // next sub-batch starts a new group of NT k-points: its headers first
-        p0((bt + 1) / BPS);
-        __syncthreads();
-      }
-      p1(bt + 1);
+      if ((bt + 1) % BPS == 0) sb_robust = p0((bt + 1) / BPS);   // next sub-batch starts a new group of NT k-points
+      if (sb_robust) p1(bt + 1, std::true_type{}); else p1(bt + 1, std::false_type{});
     }
     // ---------------- P2: TH x TD pairs per thread and slot, from buffer bt & 1 ----------------
     const double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
     const int* const ev = ev_s + (bt & 1) * SLOTS * W;
     const int2* const efs = reinterpret_cast<const int2*>(val + SLOTS * W);
+    const double* const va0 = val + tdx * 2;                          // + sl W + p 2 NTD
+    const double* const vb0 = val + WD + thx * (TH + G::PADB);        // + sl W + i
+    auto load_a = [&](double (&a)[TD], int sl) {
+#pragma unroll
+      for (int pp = 0; pp < TD / 2; ++pp) {
+        const double2 v = *reinterpret_cast<const double2*>(va0 + sl * W + pp * 2 * G::NTD);
+        a[2 * pp] = v.x; a[2 * pp + 1] = v.y;
+      }
+    };
+    auto load_b = [&](double (&bb)[HC], int sl, int i0) {
+#pragma unroll
+      for (int i = 0; i < HC; i += 2) {
+        const double2 v = *reinterpret_cast<const double2*>(vb0 + sl * W + i0 + i);
+        bb[i] = v.x; bb[i + 1] = v.y;
+      }
+    };
+    double a[TD], b0[HC];
+    load_a(a, 0);
+    load_b(b0, 0, 0);
 #pragma unroll 1
     for (int sl = 0; sl < SLOTS; ++sl) {
       const int2 ef = efs[sl];
       const int flags = ef.y;
-      if (flags & kCoopSkip) continue;
-      const int step = flags >> 8;
-      if (drift + step > kDriftLimit) {
+      double b1[HC], an[TD];
+      load_b(b1, sl, HC);                                             // second half of this slot
+      const bool fast = !(flags & (kCoopSkip | kCoopRobust));
+      if (!(flags & kCoopSkip)) {
+        const int step = flags >> 8;
+        if (drift + step > kDriftLimit) {
 #pragma unroll
-        for (int i = 0; i < TH; ++i)
+          for (int i = 0; i < TH; ++i)
 #pragma unroll
-          for (int j = 0; j < TD; ++j) {
-            const int hi = __double2hiint(accP[i][j]);
-            const int ex = (hi >> 20) - 1023;
-            myE[(i * TD + j) * NT] += ex;
-            accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
-          }
-        drift = 0;
+            for (int j = 0; j < TD; ++j) {
+              const int hi = __double2hiint(accP[i][j]);
+              const int ex = (hi >> 20) - 1023;
+              myE[(i * TD + j) * NT] += ex;
+              accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
+            }
+          drift = 0;
+        }
+        drift += step;
       }
-      drift += step;
-      const double* const va = val + sl * W + tdx * TD;
-      const double* const vb = val + sl * W + WD + thx * TH;
-      if (!(flags & kCoopRobust)) {
+      if (fast) {
         accEc += ef.x;
-        double a[TD];
 #pragma unroll
-        for (int j = 0; j < TD; j += 2) {
-          const double2 v = *reinterpret_cast<const double2*>(va + j);
-          a[j] = v.x; a[j + 1] = v.y;
-        }
-        constexpr int HC = TH < 8 ? TH : 8;
+        for (int i = 0; i < HC; ++i)
 #pragma unroll
-        for (int i0 = 0; i0 < TH; i0 += HC) {
-          double bb[HC];
+          for (int j = 0; j < TD; ++j) accP[i][j] *= (a[j] + b0[i]);
+      }
+      const int nsl = min(sl + 1, SLOTS - 1);                         // fetch the next slot's A and first B half
+      load_a(an, nsl);
+      load_b(b0, nsl, 0);
+      if (fast) {
 #pragma unroll
-          for (int i = 0; i < HC; i += 2) {
-            const double2 v = *reinterpret_cast<const double2*>(vb + i0 + i);
-            bb[i] = v.x; bb[i + 1] = v.y;
-          }
+        for (int i = 0; i < HC; ++i)
 #pragma unroll
-          for (int i = 0; i < HC; ++i)
+          for (int j = 0; j < TD; ++j) accP[HC + i][j] *= (a[j] + b1[i]);
+      } else if (flags & kCoopRobust) {
+        const double* const vb = vb0 + sl * W;
+        const int* const eb = ev + WD + thx * (TH + G::PADB) + sl * W;
 #pragma unroll
-            for (int j = 0; j < TD; ++j) accP[i0 + i][j] *= (a[j] + bb[i]);
-        }
-      } else {
-        const int* const ea = ev + sl * W + tdx * TD;
-        const int* const eb = ev + sl * W + WD + thx * TH;
+        for (int j = 0; j < TD; ++j) {
+          const int pa = sl * W + (j / 2) * (2 * G::NTD) + tdx * 2 + (j & 1);
+          const double mA = val[pa];
+          const int eA = ev[pa];
 #pragma unroll
-        for (int i = 0; i < TH; ++i) {
-          const double mB = vb[i];
-          const int eB = eb[i];
-#pragma unroll
-          for (int j = 0; j < TD; ++j) {
-            const int eA = ea[j];
+          for (int i = 0; i < TH; ++i) {
+            const int eB = eb[i];
             const int E = max(eA, eB);
-            accP[i][j] *= (scale2(va[j], eA - E) + scale2(mB, eB - E));
+            accP[i][j] *= (scale2(mA, eA - E) + scale2(vb[i], eB - E));
             myE[(i * TD + j) * NT] += E;
           }
         }
       }
+#pragma unroll
+      for (int j = 0; j < TD; ++j) a[j] = an[j];
     }
     __syncthreads();     // buffer bt & 1 may be rewritten (by P1 of sub-batch bt + 2), buffer (bt + 1) & 1 is complete
   }
