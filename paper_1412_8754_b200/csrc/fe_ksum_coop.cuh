@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const bool robust = force_robust || spread > kSpread;
       hd.eref = hi - (spread >> 1);
       int flags = robust ? (kCoopRobust | (3 << 8)) : (((spread >> 1) + 4) << 8);
-      if (!valid || !((P.mc.band_mask >> e) & 1)) flags = kCoopSkip;
+      if (!valid || !((P.mc.band_mask >> e) & 1)) { flags = kCoopSkip; hd.eref = 0; }
       any_robust |= (flags & kCoopRobust) != 0;
       hd.flags = flags;
       hdr_s[tid * NB + e] = hd;
@@ -205,9 +205,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
     int* const ev = ev_s + (bt & 1) * SLOTS * W;
     if (tid < SLOTS) reinterpret_cast<int2*>(val + SLOTS * W)[tid] = make_int2(hdr_b[tid].eref, hdr_b[tid].flags);
-    auto put = [&](int pos, double m, int e, int eref, int flags) {
+    // skip slots (k past the end of the chunk, masked band) get the neutral pair A' = 1, B' = 0: factor exactly 1
+    auto put = [&](int pos, double m, int e, int eref, int flags, double neutral) {
       if (ROB && (flags & kCoopRobust)) { val[pos] = m; ev[pos] = e; }
-      else                              val[pos] = coop_scale(m, e - eref);
+      else val[pos] = (flags & kCoopSkip) ? neutral : coop_scale(m, e - eref);
     };
     // ---- A_j = 2cosh(R_j/T) ----
 #pragma unroll 1
@@ -241,7 +242,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
         }
 #pragma unroll
         for (int u = 0; u < U; ++u)
-          if (sl0 + u < SLOTS) put((sl0 + u) * W + pos, m[u], e[u], eref[u], flags[u]);
+          if (sl0 + u < SLOTS) put((sl0 + u) * W + pos, m[u], e[u], eref[u], flags[u], 1.0);
       }
     }
     // ---- B_i = 2cosh((d0 - h_i)/T): NT / WH slots per pass ----
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 #pragma unroll
         for (int u = 0; u < U; ++u) {
           const int sl = slb + (p0i + u) * SPP;
-          if (sl < SLOTS) put(sl * W + pos, m[u], e[u], eref[u], flags[u]);
+          if (sl < SLOTS) put(sl * W + pos, m[u], e[u], eref[u], flags[u], 0.0);
         }
       }
     }
@@ -282,11 +283,43 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   __syncthreads();
 
   constexpr int HC = TH / 2;                     // the h half-tile handled between two shared-memory fetches
+  static_assert(HC % 2 == 0, "half tile");
+  // renormalisation: the exponent field of every accP moves into its integer sum (biased: 1023 per call, removed at
+  // the end through nrenorm); one shift, one shared-memory reduction and one logic op per accumulator
+  int nrenorm = 0;
+  auto renorm = [&]() {
+#pragma unroll
+    for (int i = 0; i < TH; ++i)
+#pragma unroll
+      for (int j = 0; j < TD; ++j) {
+        const int hi = __double2hiint(accP[i][j]);
+        atomicAdd(&myE[(i * TD + j) * NT], hi >> 20);
+        accP[i][j] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(accP[i][j]));
+      }
+    ++nrenorm;
+    drift = 0;
+  };
+
+  // P1 work that a thread does while it walks the slots of the CURRENT sub-batch in P2 (fused path): per slot its
+  // WD / NT values A_j of the same slot number of the NEXT sub-batch, and every SPPE-th slot one value B_i.
+  constexpr int RA = WD / NT;
+  constexpr int SPP = NT / WH, SPPE = SPP < SLOTS ? SPP : SLOTS;       // slots between two B items of a thread
+  static_assert(SLOTS % SPPE == 0 && SPPE <= 4, "fused P1 mapping");
+  double d2r[RA];
+  int posAr[RA];
+#pragma unroll
+  for (int r = 0; r < RA; ++r) { d2r[r] = d2_s[tid + r * NT]; posAr[r] = G::posA(tid + r * NT); }
+  const int ibB = tid % WH, slbB = tid / WH, posBr = G::posB(ibB);
+  const double hvB = h_s[ibB];
+
+  bool cur_robust = sb_robust;                   // robust slots among the group of the sub-batch being consumed
 #pragma unroll 1
   for (int bt = 0; bt < nbatch; ++bt) {
-    if (bt + 1 < nbatch) {
-      if ((bt + 1) % BPS == 0) sb_robust = p0((bt + 1) / BPS);   // next sub-batch starts a new group of NT k-points
-      if (sb_robust) p1(bt + 1, std::true_type{}); else p1(bt + 1, std::false_type{});
+    bool nxt_robust = cur_robust;
+    if (bt + 1 < nbatch && (bt + 1) % BPS == 0) nxt_robust = p0((bt + 1) / BPS);   // next sub-batch: new group of NT k
+    const bool fused = !cur_robust && !nxt_robust;
+    if (!fused && bt + 1 < nbatch) {
+      if (nxt_robust) p1(bt + 1, std::true_type{}); else p1(bt + 1, std::false_type{});
     }
     // ---------------- P2: TH x TD pairs per thread and slot, from buffer bt & 1 ----------------
     const double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
@@ -311,64 +344,166 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     double a[TD], b0[HC];
     load_a(a, 0);
     load_b(b0, 0, 0);
-#pragma unroll 1
-    for (int sl = 0; sl < SLOTS; ++sl) {
-      const int2 ef = efs[sl];
-      const int flags = ef.y;
-      double b1[HC], an[TD];
-      load_b(b1, sl, HC);                                             // second half of this slot
-      const bool fast = !(flags & (kCoopSkip | kCoopRobust));
-      if (!(flags & kCoopSkip)) {
-        const int step = flags >> 8;
-        if (drift + step > kDriftLimit) {
+
+    if (fused) {
+      // next sub-batch's headers and buffer ((bt + 1) may not exist: then this writes the idle buffer from stale,
+      // finite headers, which nobody reads)
+      const CoopHdr* const hdr_n = hdr_s + ((bt + 1) % BPS) * SLOTS;
+      double* const valn = buf_s + ((bt + 1) & 1) * G::BUF_DOUBLES;
+      if (tid < SLOTS) reinterpret_cast<int2*>(valn + SLOTS * W)[tid] = make_int2(hdr_n[tid].eref, hdr_n[tid].flags);
+      // The P1 chains are split in two stages that run one slot apart, so that each is short and independent of
+      // the other: stage 1 (sqrt, range reduction) of slot sl + 1 and stage 2 (polynomial, scaling, store) of slot sl.
+      double xa[RA], ta[RA];
+      int2 efn = *reinterpret_cast<const int2*>(&hdr_n[0].eref);
+      {
+        const double2 sg = *reinterpret_cast<const double2*>(&hdr_n[0].s2);
 #pragma unroll
-          for (int i = 0; i < TH; ++i)
-#pragma unroll
-            for (int j = 0; j < TD; ++j) {
-              const int hi = __double2hiint(accP[i][j]);
-              const int ex = (hi >> 20) - 1023;
-              myE[(i * TD + j) * NT] += ex;
-              accP[i][j] = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
-            }
-          drift = 0;
+        for (int r = 0; r < RA; ++r) {
+          xa[r] = sqrt_pos(fma(d2r[r], sg.y, sg.x));                  // R_j, Eq. 4 radicand          (S5)
+          ta[r] = fma(xa[r], fc.c1, MAGIC);
         }
-        drift += step;
       }
-      if (fast) {
-        accEc += ef.x;
+      double mb = 0.0, xb = 0.0, tb = 0.0;
+      int2 efb = make_int2(0, 0);
+      const double* pa = va0;                                         // this thread's A' / B' of the current slot
+      const double* pb = vb0;
+      double* pvn = valn;                                             // row of the slot being produced
+      const CoopHdr* hn = hdr_n;
+      // B' is fetched in chunks of QC values, one chunk ahead of its use (two rotating register buffers)
+      constexpr int QC = 4, NQ = TH / QC;
+      static_assert(TH % QC == 0 && NQ % 2 == 0, "chunking");
+      double bq[2][QC];
+      auto load_q = [&](double (&dst)[QC], const double* src) {
 #pragma unroll
-        for (int i = 0; i < HC; ++i)
+        for (int i = 0; i < QC; i += 2) {
+          const double2 v = *reinterpret_cast<const double2*>(src + i);
+          dst[i] = v.x; dst[i + 1] = v.y;
+        }
+      };
 #pragma unroll
-          for (int j = 0; j < TD; ++j) accP[i][j] *= (a[j] + b0[i]);
+      for (int i = 0; i < QC; ++i) bq[0][i] = b0[i];
+#pragma unroll 1
+      for (int sl0 = 0; sl0 < SLOTS; sl0 += SPPE) {
+        const int slB = slbB + (sl0 / SPPE) * SPP;                    // slot of this pass's B item
+#pragma unroll
+        for (int us = 0; us < SPPE; ++us) {
+          const int sl = sl0 + us;
+          const int2 ef = efs[sl];
+          const int step = ef.y >> 8;                                 // skip slots: step 0, Eref 0, factors 1
+          if (drift + step > kDriftLimit) renorm();
+          drift += step;
+          accEc += ef.x;
+          // ---- one straight-line block: P2 of slot sl interleaved with the P1 chains for the next sub-batch ----
+          double an[TD], ma[RA];
+          int ea[RA];
+          const int2 efa = efn;
+          const CoopHdr* const hnn = (sl + 1 < SLOTS) ? hn + 1 : hn;
+#pragma unroll
+          for (int c = 0; c < NQ; ++c) {
+            // fetch the next chunk: of this slot, or (last chunk) the first one of the next slot, and its A'
+            if (c + 1 < NQ) load_q(bq[(c + 1) & 1], pb + (c + 1) * QC);
+            else            load_q(bq[(c + 1) & 1], pb + W);
+            if (c == NQ - 2) {
+#pragma unroll
+              for (int pp = 0; pp < TD / 2; ++pp) {
+                const double2 v = *reinterpret_cast<const double2*>(pa + W + pp * 2 * G::NTD);
+                an[2 * pp] = v.x; an[2 * pp + 1] = v.y;
+              }
+            }
+            // P1 pieces, spread over the chunks
+            if (c == 0) {                                             // stage 2 of slot sl's A_j
+#pragma unroll
+              for (int r = 0; r < RA; ++r) {
+                ea[r] = exp_k(ta[r]);
+                ma[r] = exp_mant(xa[r], ta[r], fc, tab256);           // e^{R/T} = m 2^e
+              }
+              if (us == 0) {                                          // B_i of slot slB, stage 1
+                const CoopHdr* const hb = hdr_n + min(slB, SLOTS - 1);
+                xb = fabs(hb->d0 - hvB);                              // |d_i| = |d0 - h_i|
+                efb = *reinterpret_cast<const int2*>(&hb->eref);
+                tb = fma(xb, fc.c1, MAGIC);
+              }
+            }
+            if (c == 1) {                                             // stage 1 of slot sl + 1's A_j
+              const double2 sg = *reinterpret_cast<const double2*>(&hnn->s2);
+              efn = *reinterpret_cast<const int2*>(&hnn->eref);
+#pragma unroll
+              for (int r = 0; r < RA; ++r) {
+                xa[r] = sqrt_pos(fma(d2r[r], sg.y, sg.x));            // R_j, Eq. 4 radicand          (S5)
+                ta[r] = fma(xa[r], fc.c1, MAGIC);
+              }
+              if (us == 0) mb = exp_mant(xb, tb, fc, tab256);
+            }
+#pragma unroll
+            for (int i = 0; i < QC; ++i)
+#pragma unroll
+              for (int j = 0; j < TD; ++j) accP[c * QC + i][j] *= (a[j] + bq[c & 1][i]);
+          }
+#pragma unroll
+          for (int r = 0; r < RA; ++r) {
+            if (ea[r] < 28) ma[r] = cosh_fix(ma[r], ea[r]);           // + e^{-R/T} (rare)
+            pvn[posAr[r]] = (efa.y & kCoopSkip) ? 1.0 : coop_scale(ma[r], ea[r] - efa.x);
+          }
+          if (us == SPPE - 1) {                                       // B_i, stage 2
+            const int eb = exp_k(tb);
+            const double v = cosh_fix(mb, eb);
+            if (slB < SLOTS) valn[slB * W + posBr] = (efb.y & kCoopSkip) ? 0.0 : coop_scale(v, eb - efb.x);
+          }
+#pragma unroll
+          for (int j = 0; j < TD; ++j) a[j] = an[j];
+          pa += W; pb += W; pvn += W; hn = hnn;
+        }
       }
-      const int nsl = min(sl + 1, SLOTS - 1);                         // fetch the next slot's A and first B half
-      load_a(an, nsl);
-      load_b(b0, nsl, 0);
-      if (fast) {
+    } else {
+#pragma unroll 1
+      for (int sl = 0; sl < SLOTS; ++sl) {
+        const int2 ef = efs[sl];
+        const int flags = ef.y;
+        double b1[HC], an[TD];
+        load_b(b1, sl, HC);                                             // second half of this slot
+        const bool fast = !(flags & (kCoopSkip | kCoopRobust));
+        if (!(flags & kCoopSkip)) {
+          const int step = flags >> 8;
+          if (drift + step > kDriftLimit) renorm();
+          drift += step;
+        }
+        if (fast) {
+          accEc += ef.x;
 #pragma unroll
-        for (int i = 0; i < HC; ++i)
+          for (int i = 0; i < HC; ++i)
 #pragma unroll
-          for (int j = 0; j < TD; ++j) accP[HC + i][j] *= (a[j] + b1[i]);
-      } else if (flags & kCoopRobust) {
-        const double* const vb = vb0 + sl * W;
-        const int* const eb = ev + WD + thx * (TH + G::PADB) + sl * W;
+            for (int j = 0; j < TD; ++j) accP[i][j] *= (a[j] + b0[i]);
+        }
+        const int nsl = min(sl + 1, SLOTS - 1);                         // fetch the next slot's A and first B half
+        load_a(an, nsl);
+        load_b(b0, nsl, 0);
+        if (fast) {
 #pragma unroll
-        for (int j = 0; j < TD; ++j) {
-          const int pa = sl * W + (j / 2) * (2 * G::NTD) + tdx * 2 + (j & 1);
-          const double mA = val[pa];
-          const int eA = ev[pa];
+          for (int i = 0; i < HC; ++i)
 #pragma unroll
-          for (int i = 0; i < TH; ++i) {
-            const int eB = eb[i];
-            const int E = max(eA, eB);
-            accP[i][j] *= (scale2(mA, eA - E) + scale2(vb[i], eB - E));
-            myE[(i * TD + j) * NT] += E;
+            for (int j = 0; j < TD; ++j) accP[HC + i][j] *= (a[j] + b1[i]);
+        } else if (flags & kCoopRobust) {
+          const double* const vb = vb0 + sl * W;
+          const int* const eb = ev + WD + thx * (TH + G::PADB) + sl * W;
+#pragma unroll
+          for (int j = 0; j < TD; ++j) {
+            const int pa = sl * W + (j / 2) * (2 * G::NTD) + tdx * 2 + (j & 1);
+            const double mA = val[pa];
+            const int eA = ev[pa];
+#pragma unroll
+            for (int i = 0; i < TH; ++i) {
+              const int eB = eb[i];
+              const int E = max(eA, eB);
+              accP[i][j] *= (scale2(mA, eA - E) + scale2(vb[i], eB - E));
+              myE[(i * TD + j) * NT] += E;
+            }
           }
         }
-      }
 #pragma unroll
-      for (int j = 0; j < TD; ++j) a[j] = an[j];
+        for (int j = 0; j < TD; ++j) a[j] = an[j];
+      }
     }
+    cur_robust = nxt_robust;
     __syncthreads();     // buffer bt & 1 may be rewritten (by P1 of sub-batch bt + 2), buffer (bt + 1) & 1 is complete
   }
 
@@ -384,7 +519,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const int hi = __double2hiint(accP[i][j]);
       const int ex = (hi >> 20) - 1023;
       const double mant = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
-      const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] + ex);
+      const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] - 1023 * nrenorm + ex);
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(mant)));
       if (ih < P.nh && id < P.nd)
         P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = P.T * lnz;
