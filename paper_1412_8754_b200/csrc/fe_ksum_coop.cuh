@@ -312,6 +312,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   const int ibB = tid % WH, slbB = tid / WH, posBr = G::posB(ibB);
   const double hvB = h_s[ibB];
 
+  double xa[RA], ta[RA];                         // stage-1 state of the fused P1 (carried across sub-batches)
+  int2 efn = make_int2(0, 0);
+  bool have_s1 = false;
   bool cur_robust = sb_robust;                   // robust slots among the group of the sub-batch being consumed
 #pragma unroll 1
   for (int bt = 0; bt < nbatch; ++bt) {
@@ -353,16 +356,19 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       if (tid < SLOTS) reinterpret_cast<int2*>(valn + SLOTS * W)[tid] = make_int2(hdr_n[tid].eref, hdr_n[tid].flags);
       // The P1 chains are split in two stages that run one slot apart, so that each is short and independent of
       // the other: stage 1 (sqrt, range reduction) of slot sl + 1 and stage 2 (polynomial, scaling, store) of slot sl.
-      double xa[RA], ta[RA];
-      int2 efn = *reinterpret_cast<const int2*>(&hdr_n[0].eref);
-      {
+      // (stage 1 of a sub-batch's slot 0 is done at the end of the previous iteration when its headers already
+      // exist, i.e. inside a group of NT k-points: `have_s1`)
+      if (!have_s1) {
         const double2 sg = *reinterpret_cast<const double2*>(&hdr_n[0].s2);
+        efn = *reinterpret_cast<const int2*>(&hdr_n[0].eref);
 #pragma unroll
         for (int r = 0; r < RA; ++r) {
           xa[r] = sqrt_pos(fma(d2r[r], sg.y, sg.x));                  // R_j, Eq. 4 radicand          (S5)
           ta[r] = fma(xa[r], fc.c1, MAGIC);
         }
       }
+      const bool carry = (bt + 2) % BPS != 0;                         // sub-batch bt + 2 shares bt + 1's header group
+      const CoopHdr* const hdr_nn = hdr_s + ((bt + 2) % BPS) * SLOTS;
       double mb = 0.0, xb = 0.0, tb = 0.0;
       int2 efb = make_int2(0, 0);
       const double* pa = va0;                                         // this thread's A' / B' of the current slot
@@ -397,7 +403,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
           double an[TD], ma[RA];
           int ea[RA];
           const int2 efa = efn;
-          const CoopHdr* const hnn = (sl + 1 < SLOTS) ? hn + 1 : hn;
+          const CoopHdr* const hnn = (sl + 1 < SLOTS) ? hn + 1 : (carry ? hdr_nn : hn);
 #pragma unroll
           for (int c = 0; c < NQ; ++c) {
             // fetch the next chunk: of this slot, or (last chunk) the first one of the next slot, and its A'
@@ -454,7 +460,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
           pa += W; pb += W; pvn += W; hn = hnn;
         }
       }
+      have_s1 = carry;
     } else {
+      have_s1 = false;
 #pragma unroll 1
       for (int sl = 0; sl < SLOTS; ++sl) {
         const int2 ef = efs[sl];
