@@ -39,15 +39,20 @@ METRIC = "Omega evaluations/s (k-points x grid points, fp64)"
 UNIT = "k-point x (q,h,Delta) evaluations/s"
 
 # FP64-pipe instructions and flops EXECUTED per (k, band, q, h, Delta) term by the k-sum kernel as built
-# (DESIGN.md "Roofline").  factored: ncu counters smsp__sass_thread_inst_executed_op_{dfma,dadd,dmul}_pred_on of the
+# (DESIGN.md "Roofline").  coop / factored: ncu counters smsp__sass_thread_inst_executed_op_{dfma,dadd,dmul}_pred_on of the
 # cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
+    ("coop", (64, 128)): (2.382, 2.668, "ncu, profiles/r1d_ksum_coop_64x128_raw.csv (1.036 DADD + 1.060 DMUL + 0.286 DFMA)"),
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
     ("factored", (16, 4)): (4.20, 5.62, "ncu, profiles/r1c_ksum_factored_16x4_raw.csv"),
     ("direct", (4, 4)): (40.6, 61.3, "SASS count"),
     ("direct", (8, 4)): (39.4, 59.4, "SASS count"),
 }
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch from the ncu --set full capture in
+# profiles/ (a 1-q slice of the workload: 0.6 MB read, 95.5 MB written = the partial sums [ksplit][nh*nd]; the
+# launch timed here covers --q-per-step q-values and a different k-split, so this is context, not a bound: HBM is idle)
+KERNEL_TRAFFIC = {"coop": 96.1e6}
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
 PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
@@ -277,21 +282,29 @@ def main():
 
     # ---- roofline of the dominant kernel (K1 k-sum) ----
     info = F.last_launch_info()
+    info["block"] = 256
+    if info["mode"] == fe.EVAL_COOP:
+        info["block"] = next(c[4] for c in fe.coop_shapes() if (c[2], c[3]) == (info["th"], info["td"]))
     counts = KERNEL_COUNTS.get((args.mode, (info["th"], info["td"])), (None, None, None))
     k_ms = sum(ksum_ms) / len(ksum_ms)
     dfma_rate, _ = fe.fp64_peak_probe()
-    roofline = {"bound": "alu", "kernel": f"k-sum kernel ({args.mode}, tile {info['th']}x{info['td']}, grid {info['grid']} x 256)",
-                "unit": "TFLOP/s", "peak": PEAK_TFLOPS,
-                "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
-                "peak_measured_dfma_probe": 2 * dfma_rate / 1e12, "avg_launch_ms": k_ms,
-                "band_evals_per_launch": band_evals, "traffic": None,
+    # Primary roofline = FP64-pipe lane-instructions/s: a DADD or DMUL occupies an FP64 lane for a cycle exactly like a
+    # DFMA, and the kernel's pair update acc *= (A + B) has no fused form, so instructions (not flops, which count a
+    # DFMA twice) measure how busy the bounding unit is; ncu sm__pipe_fp64_cycles_active agrees (profiles/README.md).
+    roofline = {"bound": "alu", "kernel": f"k-sum kernel ({args.mode}, tile {info['th']}x{info['td']}, grid {info['grid']} x {info['block']})",
+                "unit": "Tinst/s (FP64-pipe thread-instructions: DFMA, DADD, DMUL each count 1)",
+                "peak": PEAK_DFMA_PER_S / 1e12,
+                "peak_source": "nominal: 148 SM x 64 FP64 lanes x 1.965 GHz (DESIGN.md section 6); MEASURED_PEAKS.json has no fp64 entry",
+                "peak_measured_dfma_probe": dfma_rate / 1e12, "avg_launch_ms": k_ms,
+                "band_evals_per_launch": band_evals, "traffic": KERNEL_TRAFFIC.get(args.mode),
                 "kernel_share_of_step": k_ms * len(ksum_ms) / total_ms}
     if counts[0]:
-        achieved = band_evals * counts[1] / (k_ms * 1e-3) / 1e12
-        roofline.update({"achieved": achieved, "frac": achieved / PEAK_TFLOPS,
-                         "flop_per_band_eval": counts[1], "fp64_inst_per_band_eval": counts[0], "counts_source": counts[2],
-                         "fp64_pipe_frac": band_evals * counts[0] / (k_ms * 1e-3) / PEAK_DFMA_PER_S,
-                         "frac_of_measured_dfma_peak": achieved / (2 * dfma_rate / 1e12)})
+        achieved = band_evals * counts[0] / (k_ms * 1e-3) / 1e12
+        tflops = band_evals * counts[1] / (k_ms * 1e-3) / 1e12
+        roofline.update({"achieved": achieved, "frac": achieved / (PEAK_DFMA_PER_S / 1e12),
+                         "fp64_inst_per_band_eval": counts[0], "flop_per_band_eval": counts[1], "counts_source": counts[2],
+                         "frac_of_measured_dfma_peak": achieved / (dfma_rate / 1e12),
+                         "achieved_tflops": tflops, "peak_tflops": PEAK_TFLOPS, "frac_tflops": tflops / PEAK_TFLOPS})
     else:
         roofline.update({"achieved": None, "frac": None})
 
