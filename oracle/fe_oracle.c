@@ -3,7 +3,8 @@
  *
  * Plain, slow, obviously-correct CPU evaluation of the grand potential Omega(Delta; q, h, T)
  * of PAPER.md (arXiv 1412.8754) Eq. 5 with the quasiparticle energies of Eq. 4, for the
- * one-band and the two-band (Appendix A) models, in the loop order of Algorithm 1.
+ * one-band, the two-band (Appendix A) and the three-band (Appendix B, numerically diagonalised) models, in the
+ * loop order of Algorithm 1.
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
  * may call this.  It shares NO code, header, table or constant with the CUDA path under
  * paper_1412_8754_b200/csrc (it has its own parameter struct on purpose).
@@ -49,7 +50,8 @@
 #endif
 
 typedef struct {
-    int32_t model;       /* 1: one band  E = -2 t[0] (cos kx + cos ky)   2: two-band, Appendix A  */
+    int32_t model;       /* 1: one band  E = -2 t[0] (cos kx + cos ky)   2: two-band, Appendix A
+                            3: three-band, Appendix B (hoppings in tb3, t[] unused)                */
     int32_t form_factor; /* 0: eta = eta_scale      1: eta = eta_scale cos kx cos ky */
     double  t[4];
     double  mu;
@@ -58,9 +60,10 @@ typedef struct {
     double  cond_mult;
     int32_t band_mask;   /* bit 0: band "+" (A.4 upper sign, electron-like), bit 1: band "-"      */
     int32_t const_mode;
+    double  tb3[13];     /* model 3: t1..t12 (tb3[0..11]) and eps0 (tb3[12]) of PAPER.md:242-273        */
 } feo_params;
 
-int feo_num_bands(const feo_params* p) { return p->model == 1 ? 1 : 2; }
+int feo_num_bands(const feo_params* p) { return p->model == 1 ? 1 : (p->model == 2 ? 2 : 3); }
 
 int feo_num_threads(void) {
 #ifdef _OPENMP
@@ -78,12 +81,98 @@ void feo_set_num_threads(int n) {
 #endif
 }
 
+/* Three-band orbital Hamiltonian T_k^{alpha beta} of PAPER.md:242-270, Eqs. B.1-B.6 (row-major 3x3, real and
+ * imaginary parts).  T^{12} = T^{21} real; T^{13}, T^{23} purely imaginary with T^{31} = conj(T^{13}) etc.
+ * (the equation printed twice / the missing label "B.4" are reading G14 of DESIGN.md).                          */
+void feo_three_band_matrix(const feo_params* p, double kx, double ky, double* re, double* im) {
+    const double* t = p->tb3;              /* t[i-1] = t_i */
+    const double e0 = p->tb3[12];
+    for (int i = 0; i < 9; ++i) { re[i] = 0.0; im[i] = 0.0; }
+    re[0] = 2.0 * t[1] * cos(kx) + 2.0 * t[0] * cos(ky) + 4.0 * t[2] * cos(kx) * cos(ky)
+          + 2.0 * t[10] * (cos(2.0 * kx) - cos(2.0 * ky)) + 4.0 * t[11] * cos(2.0 * kx) * cos(2.0 * ky);   /* B.1 */
+    re[4] = 2.0 * t[0] * cos(kx) + 2.0 * t[1] * cos(ky) + 4.0 * t[2] * cos(kx) * cos(ky)
+          - 2.0 * t[10] * (cos(2.0 * kx) - cos(2.0 * ky)) + 4.0 * t[11] * cos(2.0 * kx) * cos(2.0 * ky);   /* B.2 */
+    re[8] = e0 + 2.0 * t[4] * (cos(kx) + cos(ky)) + 4.0 * t[5] * cos(kx) * cos(ky)
+          + 2.0 * t[8] * (cos(2.0 * kx) + cos(2.0 * ky))
+          + 4.0 * t[9] * (cos(2.0 * kx) * cos(ky) + cos(kx) * cos(2.0 * ky));                              /* B.3 */
+    re[1] = re[3] = 4.0 * t[3] * sin(kx) * sin(ky);                                                        /* B.4 */
+    im[2] = 2.0 * t[6] * sin(kx) + 4.0 * t[7] * sin(kx) * cos(ky);   im[6] = -im[2];                       /* B.5 */
+    im[5] = 2.0 * t[6] * sin(ky) + 4.0 * t[7] * sin(ky) * cos(kx);   im[7] = -im[5];                       /* B.6 */
+}
+
+/* Eigenvalues of a 3x3 complex Hermitian matrix (row-major re/im), ascending: the numerical band diagonalisation
+ * of PAPER.md:127 ("has to be determined numerically, e.g. using ... Lapack"), Eq. 2.
+ * Cyclic complex Jacobi: for each off-diagonal pair (p, q) the unitary V = diag-phase x plane rotation that zeroes
+ * A[p][q] is formed explicitly and A <- V^H A V is computed by plain triple loops; sweeps repeat until the
+ * off-diagonal norm is below 1e-20 of the diagonal scale (at most 60).  Pinned against LAPACK zheev (numpy eigvalsh). */
+void feo_herm3_eigvals(const double* re_in, const double* im_in, double* E) {
+    double ar[3][3], ai[3][3];
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { ar[i][j] = re_in[3 * i + j]; ai[i][j] = im_in[3 * i + j]; }
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        double off = 0.0, diag = 0.0;
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {
+            const double m2 = ar[i][j] * ar[i][j] + ai[i][j] * ai[i][j];
+            if (i == j) diag += m2; else off += m2;
+        }
+        if (off <= 1e-40 * diag || off == 0.0) break;          /* |off| <= 1e-20 |diag| */
+        for (int p = 0; p < 2; ++p) for (int q = p + 1; q < 3; ++q) {
+            const double beta = hypot(ar[p][q], ai[p][q]);
+            if (beta == 0.0) continue;
+            /* A[p][q] = beta e^{i phi}.  With P = diag(.., 1_p, .., e^{-i phi}_q, ..) the (p,q) block of P^H A P is the
+             * real symmetric [[app, beta], [beta, aqq]]; the rotation J = [[c, s], [-s, c]] with
+             * t = tan(theta) = sgn(tau) / (|tau| + sqrt(1 + tau^2)), tau = (aqq - app) / (2 beta) diagonalises it. */
+            const double cphi = ar[p][q] / beta, sphi = ai[p][q] / beta;
+            const double tau = (ar[q][q] - ar[p][p]) / (2.0 * beta);
+            const double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+            const double c = 1.0 / sqrt(1.0 + t * t), s = t * c;
+            double vr[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}}, vi[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+            /* V = P J :  V[p][p] = c, V[p][q] = s, V[q][p] = -s e^{-i phi}, V[q][q] = c e^{-i phi} */
+            vr[p][p] = c;          vi[p][p] = 0.0;
+            vr[p][q] = s;          vi[p][q] = 0.0;
+            vr[q][p] = -s * cphi;  vi[q][p] = s * sphi;
+            vr[q][q] = c * cphi;   vi[q][q] = -c * sphi;
+            double br[3][3], bi[3][3], cr[3][3], ci[3][3];
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {          /* B = A V */
+                double xr = 0.0, xi = 0.0;
+                for (int k = 0; k < 3; ++k) {
+                    xr += ar[i][k] * vr[k][j] - ai[i][k] * vi[k][j];
+                    xi += ar[i][k] * vi[k][j] + ai[i][k] * vr[k][j];
+                }
+                br[i][j] = xr; bi[i][j] = xi;
+            }
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {          /* C = V^H B */
+                double xr = 0.0, xi = 0.0;
+                for (int k = 0; k < 3; ++k) {
+                    xr += vr[k][i] * br[k][j] + vi[k][i] * bi[k][j];
+                    xi += vr[k][i] * bi[k][j] - vi[k][i] * br[k][j];
+                }
+                cr[i][j] = xr; ci[i][j] = xi;
+            }
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { ar[i][j] = cr[i][j]; ai[i][j] = ci[i][j]; }
+            for (int i = 0; i < 3; ++i) ai[i][i] = 0.0;
+            ar[p][q] = ar[q][p] = 0.0; ai[p][q] = ai[q][p] = 0.0;   /* zero by construction; drop the rounding residue */
+        }
+    }
+    double e0 = ar[0][0], e1 = ar[1][1], e2 = ar[2][2], tmp;
+    if (e0 > e1) { tmp = e0; e0 = e1; e1 = tmp; }
+    if (e1 > e2) { tmp = e1; e1 = e2; e2 = tmp; }
+    if (e0 > e1) { tmp = e0; e0 = e1; e1 = tmp; }
+    E[0] = e0; E[1] = e1; E[2] = e2;
+}
+
 /* Band energies E_{eps,k} WITHOUT the -(mu + sigma h) shift.
  * one band: nearest-neighbour square lattice (BASELINE.json config 1; reading G13).
- * two band: PAPER.md:216-227, Eqs. A.1-A.4; E[0] = E_+ (electron-like), E[1] = E_- (hole-like).   */
+ * two band: PAPER.md:216-227, Eqs. A.1-A.4; E[0] = E_+ (electron-like), E[1] = E_- (hole-like).
+ * three band: eigenvalues of B.1-B.6 in ascending order, E[0] <= E[1] <= E[2] (reading G18).  */
 void feo_band_energies(const feo_params* p, double kx, double ky, double* E) {
     if (p->model == 1) {
         E[0] = -2.0 * p->t[0] * (cos(kx) + cos(ky));
+        return;
+    }
+    if (p->model == 3) {
+        double re[9], im[9];
+        feo_three_band_matrix(p, kx, ky, re, im);
+        feo_herm3_eigvals(re, im, E);
         return;
     }
     const double t1 = p->t[0], t2 = p->t[1], t3 = p->t[2], t4 = p->t[3];
@@ -133,7 +222,7 @@ static inline void acc_add(feo_acc* A, long double x) {
 int feo_omega_column(const feo_params* p, int32_t N, double T, double qx, double qy, double h,
                      const double* delta, int32_t nd, double* omega_out) {
     if (!p || !delta || !omega_out || N < 1 || nd < 1 || !(T > 0.0) || !(p->U > 0.0)) return -1;
-    if (p->model != 1 && p->model != 2) return -1;
+    if (p->model != 1 && p->model != 2 && p->model != 3) return -1;
     const int nb = feo_num_bands(p);
     const size_t nk = (size_t)N * (size_t)N;
     double* up  = (double*)malloc(sizeof(double) * nk * nb);   /* xi_{eps,k,up}        */
@@ -148,7 +237,7 @@ int feo_omega_column(const feo_params* p, int32_t N, double T, double qx, double
         for (int32_t i = 0; i < N; ++i) {
             const double kx = 2.0 * M_PI * (double)i / (double)N;
             const double ky = 2.0 * M_PI * (double)j / (double)N;
-            double Ek[2], Ekq[2];
+            double Ek[3], Ekq[3];
             feo_band_energies(p, kx, ky, Ek);
             feo_band_energies(p, -kx + qx, -ky + qy, Ekq);
             const size_t k = (size_t)j * N + i;

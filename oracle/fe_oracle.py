@@ -16,7 +16,8 @@ from . import build as _build
 class FeoParams(C.Structure):
     _fields_ = [("model", C.c_int32), ("form_factor", C.c_int32), ("t", C.c_double * 4),
                 ("mu", C.c_double), ("U", C.c_double), ("eta_scale", C.c_double),
-                ("cond_mult", C.c_double), ("band_mask", C.c_int32), ("const_mode", C.c_int32)]
+                ("cond_mult", C.c_double), ("band_mask", C.c_int32), ("const_mode", C.c_int32),
+                ("tb3", C.c_double * 13)]
 
 
 _lib = None
@@ -35,6 +36,10 @@ def lib():
         L.feo_set_num_threads.argtypes = [C.c_int]
         L.feo_band_energies.argtypes = [pp, C.c_double, C.c_double, dp]
         L.feo_band_energies.restype = None
+        L.feo_three_band_matrix.argtypes = [pp, C.c_double, C.c_double, dp, dp]
+        L.feo_three_band_matrix.restype = None
+        L.feo_herm3_eigvals.argtypes = [dp, dp, dp]
+        L.feo_herm3_eigvals.restype = None
         L.feo_eta.argtypes = [pp, C.c_double, C.c_double]
         L.feo_eta.restype = C.c_double
         L.feo_quasiparticle.argtypes = [C.c_double, C.c_double, C.c_double, dp, dp]
@@ -60,6 +65,8 @@ def _params(p: dict) -> FeoParams:
         s.t[i] = p["t"][i]
     s.mu, s.U, s.eta_scale, s.cond_mult = p["mu"], p["U"], p["eta_scale"], p["cond_mult"]
     s.band_mask, s.const_mode = p["band_mask"], p["const_mode"]
+    for i, v in enumerate(p.get("tb3", ())):
+        s.tb3[i] = v
     return s
 
 
@@ -77,9 +84,26 @@ def set_num_threads(n: int) -> None:
 
 def band_energies(p: dict, kx: float, ky: float) -> np.ndarray:
     sp = _params(p)
-    out = np.zeros(2)
+    out = np.zeros(3)
     lib().feo_band_energies(C.byref(sp), kx, ky, _dptr(out))
-    return out[: (1 if p["model"] == 1 else 2)]
+    return out[: {1: 1, 2: 2, 3: 3}[p["model"]]]
+
+
+def three_band_matrix(p: dict, kx: float, ky: float) -> np.ndarray:
+    """Complex 3x3 orbital Hamiltonian T_k of Eqs. B.1-B.6."""
+    sp = _params(p)
+    re, im = np.zeros(9), np.zeros(9)
+    lib().feo_three_band_matrix(C.byref(sp), kx, ky, _dptr(re), _dptr(im))
+    return (re + 1j * im).reshape(3, 3)
+
+
+def herm3_eigvals(a) -> np.ndarray:
+    """Ascending eigenvalues of a 3x3 complex Hermitian matrix (the oracle's Jacobi routine)."""
+    a = np.asarray(a, dtype=np.complex128).reshape(3, 3)
+    re, im = np.ascontiguousarray(a.real).reshape(-1), np.ascontiguousarray(a.imag).reshape(-1)
+    out = np.zeros(3)
+    lib().feo_herm3_eigvals(_dptr(re), _dptr(im), _dptr(out))
+    return out
 
 
 def eta(p: dict, kx: float, ky: float) -> float:

@@ -21,22 +21,31 @@ import numpy as np
 TWO_BAND_T = (-1.0, 1.3, -0.85, -0.85)
 TWO_BAND_MU = 1.54
 
+# PAPER.md:273 (Appendix B): three-band model of Daghofer et al., hoppings in eV, t1..t12 then eps0; n = 4 at mu = 0.4748.
+THREE_BAND_T = (-0.08, 0.1825, 0.08375, -0.03, 0.15, 0.15, -0.12, 0.06, 0.0, -0.024, -0.01, 0.0275, 0.75)
+THREE_BAND_MU = 0.4748
+
 MODEL_ONE_BAND = 1
 MODEL_TWO_BAND = 2
+MODEL_THREE_BAND = 3
+NBANDS = {MODEL_ONE_BAND: 1, MODEL_TWO_BAND: 2, MODEL_THREE_BAND: 3}
 FORM_S = 0        # eta = 1                  (homogeneous BCS)
 FORM_SPM = 1      # eta = cos kx cos ky      (s+-)
 
 
 def model_params(model=MODEL_TWO_BAND, form_factor=FORM_SPM, t=TWO_BAND_T, mu=TWO_BAND_MU,
-                 U=2.0, eta_scale=1.0, cond_mult=None, band_mask=None, const_mode=0):
+                 U=2.0, eta_scale=1.0, cond_mult=None, band_mask=None, const_mode=0, tb3=None):
     """Plain dict mirrored field-by-field by both C structs (fe_model_params / feo_params)."""
-    nb = 1 if model == MODEL_ONE_BAND else 2
+    nb = NBANDS[model]
+    if model == MODEL_THREE_BAND:
+        t, tb3 = (), (THREE_BAND_T if tb3 is None else tb3)
+    tb3 = tuple(float(x) for x in (tb3 or ())) + (0.0,) * (13 - len(tb3 or ()))
     t4 = tuple(float(x) for x in t) + (0.0,) * (4 - len(t))
     return dict(model=int(model), form_factor=int(form_factor), t=t4, mu=float(mu), U=float(U),
                 eta_scale=float(eta_scale),
                 cond_mult=float(nb if cond_mult is None else cond_mult),
                 band_mask=int((1 << nb) - 1 if band_mask is None else band_mask),
-                const_mode=int(const_mode))
+                const_mode=int(const_mode), tb3=tb3)
 
 
 @dataclass
@@ -66,7 +75,7 @@ class Workload:
 
     @property
     def nbands(self):
-        return 1 if self.params["model"] == MODEL_ONE_BAND else 2
+        return NBANDS[self.params["model"]]
 
     def k_param_evals(self):
         """k-point x parameter evaluations per temperature (the unit of BASELINE.json's metric)."""
