@@ -495,7 +495,7 @@ def test_oracle_rejects_bad_input(oracle):
     with pytest.raises(ValueError):
         oracle.omega_column(dict(TWO, U=0.0), 8, 0.1, (0, 0), 0.0, [0.1])
     with pytest.raises(ValueError):
-        oracle.omega_column(dict(TWO, model=3), 8, 0.1, (0, 0), 0.0, [0.1])
+        oracle.omega_column(dict(TWO, model=4), 8, 0.1, (0, 0), 0.0, [0.1])          # models are 1, 2, 3
 
 
 def test_survey_anchor_config1(oracle):
