@@ -43,6 +43,11 @@ extern "C" {
 #define FE_MODEL_ONE_BAND 1 /* E_k = -2 t[0] (cos kx + cos ky): nearest-neighbour square lattice (BCS use) */
 #define FE_MODEL_TWO_BAND 2 /* Raghu et al. two-orbital model, Eqs. A.1-A.4, t[0..3] = t1..t4;
                                band 0 = E_+ (electron-like), band 1 = E_- (hole-like)             */
+#define FE_MODEL_THREE_BAND 3 /* Daghofer et al. three-orbital model, Eqs. B.1-B.6, hoppings in tb3[];
+                                 the 3x3 complex-Hermitian T_k is diagonalised numerically on the device and the
+                                 eigenvalues are stored in per-q tables in HBM, as the paper proposes for more than two
+                                 bands; band e = e-th eigenvalue in ascending order.
+                                 FE_EVAL_COOP only.                                                                */
 #define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
 #define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
 
@@ -78,6 +83,7 @@ typedef struct {
   int32_t const_mode;  /* 0: constant of Eq. 5 = sum_k xi_{eps,-k+q,dn} (what the Bogoliubov transformation
                              of Eq. 3 gives for any q)   1: sum_k xi_{eps,k,dn} (Eq. 5 as printed; equal for
                              on-grid q)                                                                     */
+  double  tb3[13];     /* FE_MODEL_THREE_BAND: t1..t12 = tb3[0..11], eps0 = tb3[12]; else ignored */
 } fe_model_params;
 
 /* Create a handle for an N x N k-grid at temperature T (k_B = 1, energies in units of |t1|).

@@ -8,8 +8,10 @@
 #include <new>
 
 #include "../../include/fe.h"
+#define FE_PLAIN_KERNELS
 #include "fe_kernels.cuh"
-#include "fe_ksum_coop.cuh"
+#include "fe_bands3.cuh"
+#include "fe_launch.h"
 
 namespace {
 
@@ -69,6 +71,9 @@ struct fe_handle {
   size_t partial_cap = 0;
   double* d_spart = nullptr;
   size_t spart_cap = 0;
+  double* d_etab = nullptr;    // three-band model: [1 + nq][3][N*N] eigenvalue tables
+  size_t etab_cap = 0;
+  bool etab_base_valid = false;   // table 0 (unshifted grid) already computed for this handle
   double* d_omega = nullptr;   // fe_scan_host only
   size_t omega_cap = 0;
   void* d_res = nullptr;       // fe_scan_host: idx | dstar | ostar
@@ -86,13 +91,27 @@ struct fe_handle {
 
 namespace {
 
-int nbands(const fe_model_params& p) { return p.model == FE_MODEL_ONE_BAND ? 1 : 2; }
+int nbands(const fe_model_params& p) {
+  return p.model == FE_MODEL_ONE_BAND ? 1 : (p.model == FE_MODEL_TWO_BAND ? 2 : 3);
+}
+
+// |E_k| <= Wb for every band and k (Gershgorin on the orbital matrix): used by the range guards of the k-sum.
+double band_half_width(const fe_model_params& mp) {
+  if (mp.model == FE_MODEL_ONE_BAND) return 4.0 * fabs(mp.t[0]);
+  if (mp.model == FE_MODEL_TWO_BAND)
+    return 2.0 * (fabs(mp.t[0]) + fabs(mp.t[1])) + 4.0 * fabs(mp.t[2]) + 4.0 * fabs(mp.t[3]);
+  const double* t = mp.tb3;   // t[i-1] = t_i
+  const double d12 = 2.0 * (fabs(t[0]) + fabs(t[1])) + 4.0 * fabs(t[2]) + 4.0 * fabs(t[10]) + 4.0 * fabs(t[11]);
+  const double d3 = fabs(t[12]) + 4.0 * fabs(t[4]) + 4.0 * fabs(t[5]) + 4.0 * fabs(t[8]) + 8.0 * fabs(t[9]);
+  const double o12 = 4.0 * fabs(t[3]), o3 = 2.0 * fabs(t[6]) + 4.0 * fabs(t[7]);
+  return fmax(d12 + o12 + o3, d3 + 2.0 * o3);
+}
 
 bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
 
 int validate_params(const fe_model_params* p, int32_t N, double T) {
   if (!p) { snprintf(g_errbuf, sizeof g_errbuf, "params is NULL"); return FE_EINVAL; }
-  if (p->model != FE_MODEL_ONE_BAND && p->model != FE_MODEL_TWO_BAND) {
+  if (p->model != FE_MODEL_ONE_BAND && p->model != FE_MODEL_TWO_BAND && p->model != FE_MODEL_THREE_BAND) {
     snprintf(g_errbuf, sizeof g_errbuf, "unknown model %d", p->model); return FE_EINVAL; }
   if (p->form_factor != FE_FORM_S && p->form_factor != FE_FORM_SPM) {
     snprintf(g_errbuf, sizeof g_errbuf, "unknown form_factor %d", p->form_factor); return FE_EINVAL; }
@@ -102,8 +121,10 @@ int validate_params(const fe_model_params* p, int32_t N, double T) {
   if (!finite_pos(T)) { snprintf(g_errbuf, sizeof g_errbuf, "T must be finite and > 0"); return FE_EINVAL; }
   if (!finite_pos(p->U)) { snprintf(g_errbuf, sizeof g_errbuf, "U must be finite and > 0"); return FE_EINVAL; }
   const int nb = nbands(*p);
-  for (int i = 0; i < (nb == 1 ? 1 : 4); ++i)
+  for (int i = 0; i < (nb == 1 ? 1 : 4) && nb < 3; ++i)
     if (!isfinite(p->t[i])) { snprintf(g_errbuf, sizeof g_errbuf, "t[%d] is not finite", i); return FE_EINVAL; }
+  for (int i = 0; i < 13 && nb == 3; ++i)
+    if (!isfinite(p->tb3[i])) { snprintf(g_errbuf, sizeof g_errbuf, "tb3[%d] is not finite", i); return FE_EINVAL; }
   if (!isfinite(p->mu) || !isfinite(p->eta_scale) || !isfinite(p->cond_mult)) {
     snprintf(g_errbuf, sizeof g_errbuf, "mu, eta_scale, cond_mult must be finite"); return FE_EINVAL; }
   if (p->band_mask < 0 || p->band_mask >= (1 << nb)) {
@@ -127,6 +148,8 @@ ModelConsts make_consts(const fe_model_params& p) {
   ModelConsts mc;
   if (p.model == FE_MODEL_ONE_BAND) {
     mc.tp = -2.0 * p.t[0]; mc.tm = 0; mc.t3x4 = 0; mc.t4x4 = 0;
+  } else if (p.model == FE_MODEL_THREE_BAND) {
+    mc.tp = 0; mc.tm = 0; mc.t3x4 = 0; mc.t4x4 = 0;      // bands come from the tables (fe_bands3.cuh)
   } else {
     mc.tp = -(p.t[0] + p.t[1]);
     mc.tm = -(p.t[0] - p.t[1]);
@@ -135,21 +158,6 @@ ModelConsts make_consts(const fe_model_params& p) {
   }
   mc.mu = p.mu; mc.eta_scale = p.eta_scale; mc.band_mask = p.band_mask; mc.const_mode = p.const_mode;
   return mc;
-}
-
-FactoredConsts make_factored(double T) {
-  FactoredConsts fc;
-  const long double ln2 = 0.693147180559945309417232121458176568L;
-  const long double c2 = (long double)T * ln2 / 256.0L;
-  fc.c1 = (double)(256.0L / ((long double)T * ln2));
-  fc.c2hi = (double)c2;
-  fc.c2lo = (double)(c2 - (long double)fc.c2hi);
-  const long double beta = 1.0L / (long double)T;
-  fc.b1 = (double)beta;
-  fc.b2 = (double)(beta * beta / 2.0L);
-  fc.b3 = (double)(beta * beta * beta / 6.0L);
-  fc.b4 = (double)(beta * beta * beta * beta / 24.0L);
-  return fc;
 }
 
 template <typename T>
@@ -219,63 +227,23 @@ int choose_tile_mode(int forced_tile, int mode, int nh, int nd) {
 }
 
 
-template <int NB, int FORM, int TH, int TD>
-cudaError_t launch_ksum_mode(int mode, int grid, cudaStream_t st, const KsumParams& P) {
-  if (mode == FE_EVAL_WINDOWED)    fe_ksum_kernel<NB, FORM, TH, TD, 1><<<grid, kThreads, 0, st>>>(P);
-  else if (mode == FE_EVAL_DIRECT) fe_ksum_kernel<NB, FORM, TH, TD, 0><<<grid, kThreads, 0, st>>>(P);
-  else                             fe_ksum_factored_kernel<NB, FORM, TH, TD><<<grid, kFThreads, 0, st>>>(P, make_factored(P.T));
-  return cudaGetLastError();
-}
-
-template <int TH, int TD>
-cudaError_t launch_ksum_tile(int nb, int form, int mode, int grid, cudaStream_t st, const KsumParams& P) {
-  if (nb == 1) return form == 0 ? launch_ksum_mode<1, 0, TH, TD>(mode, grid, st, P)
-                                : launch_ksum_mode<1, 1, TH, TD>(mode, grid, st, P);
-  return form == 0 ? launch_ksum_mode<2, 0, TH, TD>(mode, grid, st, P)
-                   : launch_ksum_mode<2, 1, TH, TD>(mode, grid, st, P);
-}
-
 cudaError_t launch_ksum(int tile, int nb, int form, int mode, int grid, cudaStream_t st, const KsumParams& P) {
-  switch (tile) {
-    case 0: return launch_ksum_tile<8, 4>(nb, form, mode, grid, st, P);
-    case 1: return launch_ksum_tile<4, 4>(nb, form, mode, grid, st, P);
-    case 2: return launch_ksum_tile<2, 8>(nb, form, mode, grid, st, P);
-    case 3: return launch_ksum_tile<1, 8>(nb, form, mode, grid, st, P);
-    case 4: return launch_ksum_tile<16, 2>(nb, form, mode, grid, st, P);
-    default: return launch_ksum_tile<16, 4>(nb, form, mode, grid, st, P);
+  switch (tile) {      // kTiles order
+    case 0: return launch_ksum_tile_0(nb, form, mode, grid, st, P);
+    case 1: return launch_ksum_tile_1(nb, form, mode, grid, st, P);
+    case 2: return launch_ksum_tile_2(nb, form, mode, grid, st, P);
+    case 3: return launch_ksum_tile_3(nb, form, mode, grid, st, P);
+    case 4: return launch_ksum_tile_4(nb, form, mode, grid, st, P);
+    default: return launch_ksum_tile_5(nb, form, mode, grid, st, P);
   }
-}
-
-
-// ---- K1c (block-cooperative factored kernel) -------------------------------------------------------
-template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
-cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
-  using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
-  auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB>;
-  static bool attr_set = false;     // per instantiation; the attribute is sticky for the function
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
-  kern<<<grid, G::NT, G::smem_bytes, st>>>(P);
-  return cudaGetLastError();
-}
-
-template <int TH, int TD, int LH, int NW, int KB, int MINB>
-cudaError_t launch_coop_shape(int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
-  if (nb == 1) return form == 0 ? launch_coop_inst<1, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
-                                : launch_coop_inst<1, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
-  return form == 0 ? launch_coop_inst<2, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
-                   : launch_coop_inst<2, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
 }
 
 cudaError_t launch_coop(int shape, int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
-  switch (shape) {
-    case 0: return launch_coop_shape<16, 4, 4, 4, 4, 2>(nb, form, grid, st, P);
-    case 1: return launch_coop_shape<16, 4, 1, 4, 2, 2>(nb, form, grid, st, P);
-    case 2: return launch_coop_shape<8, 4, 4, 4, 4, 3>(nb, form, grid, st, P);
-    default: return launch_coop_shape<8, 4, 1, 4, 2, 2>(nb, form, grid, st, P);
+  switch (shape) {     // kCoopShapes order
+    case 0: return launch_coop_shape_0(nb, form, grid, st, P);
+    case 1: return launch_coop_shape_1(nb, form, grid, st, P);
+    case 2: return launch_coop_shape_2(nb, form, grid, st, P);
+    default: return launch_coop_shape_3(nb, form, grid, st, P);
   }
 }
 
@@ -292,6 +260,7 @@ int choose_coop_shape(const fe_handle* h, int nh, int nd) {
   int best = 0; double best_cost = 1e300;
   for (int t = 0; t < kNumCoopShapes; ++t) {
     const CoopShape& s = kCoopShapes[t];
+    if (h->nb == 3 && s.lh != 4) continue;
     const int wh = s.th * s.lh, wd = s.td * s.nw * (32 / s.lh);
     const double padded = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd);
     const double cost = padded * coop_shape_cost(s);
@@ -316,9 +285,13 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
   int mode = h->mode;
   int cshape = 0;
+  if (h->nb == 3 && mode != FE_EVAL_COOP) {
+    snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND supports FE_EVAL_COOP only"); return FE_EINVAL; }
   if (mode == FE_EVAL_COOP) {
     cshape = choose_coop_shape(h, nh, nd);
-    if (h->coop_shape == 0) {
+    if (h->nb == 3 && kCoopShapes[cshape].lh != 4) {
+      snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND needs a coop shape with 4 lanes along h"); return FE_EINVAL; }
+    if (h->coop_shape == 0 && h->nb < 3) {
       const CoopShape& cs = kCoopShapes[cshape];
       const int wh = cs.th * cs.lh, wd = cs.td * cs.nw * (32 / cs.lh);
       const double coop_cost = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd) *
@@ -400,8 +373,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     // Range guards of the factored kernel: binary exponents x/(T ln2) are summed in int32 per thread, and the
     // range reduction needs x/T * 64/ln2 < 2^37.  |E_k| <= W, so R <= W + |mu| + |Delta eta|, |d| <= W + |h|.
     const fe_model_params& mp = h->p;
-    const double Wb = mp.model == FE_MODEL_ONE_BAND ? 4.0 * fabs(mp.t[0])
-                    : 2.0 * (fabs(mp.t[0]) + fabs(mp.t[1])) + 4.0 * fabs(mp.t[2]) + 4.0 * fabs(mp.t[3]);
+    const double Wb = band_half_width(mp);
     double hmax = 0, dmax = 0;
     for (int i = 0; i < nh; ++i) hmax = fmax(hmax, fabs(h_list[i]));
     for (int i = 0; i < nd; ++i) dmax = fmax(dmax, fabs(delta[i]));
@@ -470,6 +442,11 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   const int srpc = (N + nschunk - 1) / nschunk;
   nschunk = (N + srpc - 1) / srpc;
   if ((rc = ensure(h->d_spart, h->spart_cap, (size_t)nq * nschunk))) return rc;
+  if (h->nb == 3) {
+    const size_t need = (size_t)(1 + nq) * 3 * N * N;
+    if (need > h->etab_cap || !h->d_etab) h->etab_base_valid = false;      // reallocation drops table 0
+    if ((rc = ensure(h->d_etab, h->etab_cap, need))) return rc;
+  }
 
   P.coltab = h->d_coltab; P.rowtab = h->d_rowtab; P.h = d_h; P.d2 = d_d2; P.htile = d_htile; P.tabs = h->d_tabs;
   P.partial = h->d_partial;
@@ -481,7 +458,22 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     FE_CUDA(cudaGetLastError());
     h->launches++;
   }
-  {
+  if (h->nb == 3) {
+    // KB: numerical band diagonalisation into the per-q tables (table 0 = unshifted grid, once per handle)
+    Band3Consts bc;
+    for (int i = 0; i < 12; ++i) bc.t[i] = h->p.tb3[i];
+    bc.e0 = h->p.tb3[12];
+    const int y0 = h->etab_base_valid ? 1 : 0;
+    dim3 g((unsigned)(((size_t)N * N + 255) / 256), (unsigned)(1 + nq - y0));
+    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, h->d_etab);
+    FE_CUDA(cudaGetLastError());
+    h->etab_base_valid = true;
+    h->launches++;
+    dim3 gs(nschunk, nq);
+    fe_ssum3_kernel<<<gs, kThreads, 0, st>>>(P.mc, N, srpc, h->d_etab, h->d_spart);
+    FE_CUDA(cudaGetLastError());
+    h->launches++;
+  } else {
     dim3 g(nschunk, nq);
     if (h->nb == 1) fe_ssum_kernel<1><<<g, kThreads, 0, st>>>(P.mc, N, srpc, h->d_coltab, h->d_rowtab, h->d_spart);
     else            fe_ssum_kernel<2><<<g, kThreads, 0, st>>>(P.mc, N, srpc, h->d_coltab, h->d_rowtab, h->d_spart);
@@ -495,7 +487,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     h->last_info[0] = cs.th * cs.lh; h->last_info[1] = cs.td * cs.nw * (32 / cs.lh);     // block tile WH x WD
     h->last_info[5] = (int32_t)(CP.kc < 2147483647ULL ? CP.kc : 2147483647ULL);          // k-points per chunk
     CP.coltab = h->d_coltab; CP.rowtab = h->d_rowtab; CP.h = d_h; CP.d2 = d_d2; CP.tabs = h->d_tabs;
-    CP.partial = h->d_partial;
+    CP.partial = h->d_partial; CP.etab = h->d_etab;
   }
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
   if (coop) FE_CUDA(launch_coop(cshape, h->nb, h->p.form_factor, (int)grid_ll, st, CP));
@@ -737,7 +729,7 @@ int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, d
 void fe_destroy(fe_handle* h) {
   if (!h) return;
   cudaFree(h->d_tabs); cudaFree(h->d_coltab); cudaFree(h->d_rowtab); cudaFree(h->d_partial);
-  cudaFree(h->d_spart); cudaFree(h->d_omega); cudaFree(h->d_res);
+  cudaFree(h->d_spart); cudaFree(h->d_etab); cudaFree(h->d_omega); cudaFree(h->d_res);
   for (auto& s : h->slots) {
     if (s.pending && s.ev) cudaEventSynchronize(s.ev);
     if (s.host) cudaFreeHost(s.host);

@@ -86,6 +86,7 @@ __device__ __forceinline__ void band_energies(const ModelConsts& mc, double cx, 
   }
 }
 
+#ifdef FE_PLAIN_KERNELS   // non-template kernels live in ONE translation unit (fe_api.cu); see build.py
 // ---------------------------------------------------------------------------------------------------
 // K0: trig tables.  One thread per (iq, i).  Angles are formed exactly as k = 2 pi i / N and k - q in fp64
 // and evaluated with CUDA's sincos (<= 2 ulp); E is even, so E(-k+q) = E(k-q).
@@ -103,6 +104,7 @@ __global__ void fe_trig_kernel(int N, int nq, const double* __restrict__ q_xy, d
   sincos(k - q_xy[2 * iq + 1], &s1, &c1);
   rowtab[idx] = make_double4(c0, s0, c1, s1);
 }
+#endif  // FE_PLAIN_KERNELS
 
 // Fixed-order block sum of one double per thread; result valid in thread 0.
 __device__ __forceinline__ double warp_sum(double v) {
@@ -592,6 +594,7 @@ __global__ void __launch_bounds__(kFThreads, (TH * TD > 32 ? 2 : FE_FACTORED_MIN
   }
 }
 
+#ifdef FE_PLAIN_KERNELS
 // ---------------------------------------------------------------------------------------------------
 // K2: Omega[o] = (S[iq] - sum_c partial[c][o]) + condc * Delta^2, chunks and S-chunks summed in index order.
 // ---------------------------------------------------------------------------------------------------
@@ -671,5 +674,6 @@ __global__ void fe_math_probe_kernel(int which, int n, const double* __restrict_
   if (i >= n) return;
   y[i] = which == 0 ? exp_nonpos(x[i], tabs) : log_1p_w(x[i], tabs);
 }
+#endif  // FE_PLAIN_KERNELS
 
 }  // namespace fe

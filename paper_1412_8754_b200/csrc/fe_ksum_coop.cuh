@@ -8,7 +8,8 @@
 // is half of its FP64 work.  Here a block owns ONE (h, Delta) block tile of WH x WD values and a contiguous chunk of
 // k-points, and its threads share the exponentials through shared memory:
 //
-//   P0  (once per NT k-points, one k per thread)  dispersion A.1-A.4 at k and k-q, s, d0, eta^2 per band, and the
+//   P0  (once per NT k-points, one k per thread)  dispersion A.1-A.4 at k and k-q (three-band model: the
+//       eigenvalues of B.1-B.6 read from the per-q tables of fe_bands3.cuh), s, d0, eta^2 per band, and the
 //       block tile's exponent bounds -> a 32-byte header per (k, band) "slot": {s^2, eta^2, d0, Eref, flags}.
 //   P1  (per sub-batch of KB k-points)  the SLOTS x (WD + WH) exponentials A_j, B_i: a thread keeps a fixed Delta_j
 //       (and a fixed h_i) and walks the slots, four independent sqrt / exp chains at a time; results are scaled by
@@ -48,6 +49,7 @@ struct CoopParams {
   const double* h;                     // [nh]
   const double* d2;                    // [nd]  Delta^2
   const MathTabs* tabs;
+  const double* etab;                  // NB == 3 only: [1 + nq][3][N*N] band tables, y = 0: E(k), 1 + iq: E(k - q)
   double* partial;                     // [ksplit][nq*nh*nd]
 };
 
@@ -161,8 +163,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     const double4 ct = P.coltab[(size_t)iq * P.N + col];
     const double4 rr = P.rowtab[(size_t)iq * P.N + row];
     double Ek[NB], Eq[NB];
-    band_energies<NB>(P.mc, ct.x, ct.y, rr.x, rr.y, Ek);     // E(k)                       (S2)
-    band_energies<NB>(P.mc, ct.z, ct.w, rr.z, rr.w, Eq);     // E(k - q) = E(-k + q)
+    if constexpr (NB == 3) {                                 // three-band model: numerically diagonalised bands
+#pragma unroll                                               // from the per-q tables in HBM
+      for (int e = 0; e < 3; ++e) {
+        Ek[e] = P.etab[(size_t)e * P.nk + kk];
+        Eq[e] = P.etab[((size_t)(1 + iq) * 3 + e) * P.nk + kk];
+      }
+    } else {
+      band_energies<NB>(P.mc, ct.x, ct.y, rr.x, rr.y, Ek);   // E(k)                       (S2)
+      band_energies<NB>(P.mc, ct.z, ct.w, rr.z, rr.w, Eq);   // E(k - q) = E(-k + q)
+    }
     double g2 = P.mc.eta_scale;                              // eta(k)                     (S4)
     if (FORM == 1) g2 *= ct.x * rr.x;
     g2 *= g2;

@@ -1,0 +1,44 @@
+// fe_launch_coop.cu -- K1c instantiations of ONE block shape.  Compiled once per shape by build.py with
+// -DFE_COOP_ID=i -DFE_COOP_TH=.. -DFE_COOP_TD=.. -DFE_COOP_LH=.. -DFE_COOP_NW=.. -DFE_COOP_KB=.. -DFE_COOP_MINB=..
+#include "../../include/fe.h"
+#include "fe_launch.h"
+
+namespace fe {
+namespace {
+
+template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
+cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
+  using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
+  auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB>;
+  static bool attr_set = false;     // per instantiation; the attribute is sticky for the function
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  kern<<<grid, G::NT, G::smem_bytes, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int TH, int TD, int LH, int NW, int KB, int MINB>
+cudaError_t launch_coop_shape(int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
+  if constexpr (LH == 4) {          // three-band model: the LH = 4 shapes only (fused-P1 slot mapping, fe_ksum_coop.cuh)
+    if (nb == 3) return form == 0 ? launch_coop_inst<3, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
+                                  : launch_coop_inst<3, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
+  }
+  if (nb == 3) return cudaErrorInvalidConfiguration;
+  if (nb == 1) return form == 0 ? launch_coop_inst<1, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
+                                : launch_coop_inst<1, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
+  return form == 0 ? launch_coop_inst<2, 0, TH, TD, LH, NW, KB, MINB>(grid, st, P)
+                   : launch_coop_inst<2, 1, TH, TD, LH, NW, KB, MINB>(grid, st, P);
+}
+
+}  // namespace
+
+#define FE_CAT2(a, b) a##b
+#define FE_CAT(a, b) FE_CAT2(a, b)
+cudaError_t FE_CAT(launch_coop_shape_, FE_COOP_ID)(int nb, int form, int grid, cudaStream_t st, const CoopParams& P) {
+  return launch_coop_shape<FE_COOP_TH, FE_COOP_TD, FE_COOP_LH, FE_COOP_NW, FE_COOP_KB, FE_COOP_MINB>(nb, form, grid, st, P);
+}
+
+}  // namespace fe

@@ -30,7 +30,8 @@ class FeError(RuntimeError):
 class ModelParams(C.Structure):
     _fields_ = [("model", C.c_int32), ("form_factor", C.c_int32), ("t", C.c_double * 4),
                 ("mu", C.c_double), ("U", C.c_double), ("eta_scale", C.c_double),
-                ("cond_mult", C.c_double), ("band_mask", C.c_int32), ("const_mode", C.c_int32)]
+                ("cond_mult", C.c_double), ("band_mask", C.c_int32), ("const_mode", C.c_int32),
+                ("tb3", C.c_double * 13)]
 
 
 _lib = None
@@ -109,6 +110,8 @@ def make_params(p: dict) -> ModelParams:
         s.t[i] = p["t"][i]
     s.mu, s.U, s.eta_scale, s.cond_mult = p["mu"], p["U"], p["eta_scale"], p["cond_mult"]
     s.band_mask, s.const_mode = p["band_mask"], p["const_mode"]
+    for i, v in enumerate(p.get("tb3", ())):
+        s.tb3[i] = v
     return s
 
 

@@ -158,6 +158,23 @@ def interior_minimum(N=128, U=5.0, T=0.001, nq=8, nh=16, nd=256):
                     np.linspace(0.0, 0.3, nh), np.linspace(0.0, 0.4, nd), "interior-minimum grid")
 
 
+def three_band(N=256, U=1.5, T=0.001, nq=8, nh=16, nd=128, qdir="axis"):
+    """the three-band model of Appendix B (hoppings in eV, mu = 0.4748) with s+-
+    pairing.  U = 1.5 eV gives Delta* ~ 0.044 eV at h = 0 and first-order jumps to Delta* = 0 for h in [0.02, 0.04]."""
+    v = np.linspace(0.0, 0.2 * math.pi, nq)
+    return Workload(f"B3_U{U:g}_N{N}_T{T:g}", model_params(model=MODEL_THREE_BAND, mu=THREE_BAND_MU, U=U), N, (T,),
+                    _q_axis(v) if qdir == "axis" else _q_diag(v),
+                    np.linspace(0.0, 0.06, nh), np.linspace(0.0, 0.15, nd), "three-band FFLO scan")
+
+
+def ragged3(seed=11, N=37, nq=3, nh=5, nd=19):
+    """Awkward sizes for the three-band model: odd N, off-grid q of both signs, negative h / Delta."""
+    rng = np.random.default_rng(seed)
+    return Workload(f"ragged3_s{seed}_N{N}", model_params(model=MODEL_THREE_BAND, mu=THREE_BAND_MU, U=1.3), N, (0.002,),
+                    rng.uniform(-0.6, 0.6, size=(nq, 2)), np.sort(rng.uniform(-0.02, 0.06, size=nh)),
+                    np.sort(rng.uniform(-0.02, 0.16, size=nd)), "ragged sizes, three bands")
+
+
 def ragged(seed=7, N=45, nq=3, nh=5, nd=37, model=MODEL_TWO_BAND):
     """Deliberately awkward sizes: odd N, list lengths that divide no tile, off-grid q, negative h/Delta."""
     rng = np.random.default_rng(seed)

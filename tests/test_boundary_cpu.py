@@ -40,9 +40,11 @@ def test_no_python_level_fallback_in_binding():
 def test_param_struct_matches_header_layout():
     from paper_1412_8754_b200 import fe
     s = fe.make_params(W.model_params(U=3.5, const_mode=1, band_mask=2, cond_mult=1.0))
-    assert C.sizeof(s) == 4 + 4 + 32 + 8 * 4 + 4 + 4      # 80 bytes, no hidden padding surprises
+    assert C.sizeof(s) == 4 + 4 + 32 + 8 * 4 + 4 + 4 + 8 * 13     # 184 bytes, no hidden padding surprises
     assert (s.model, s.form_factor, s.band_mask, s.const_mode) == (2, 1, 2, 1)
     assert list(s.t) == list(W.TWO_BAND_T) and s.U == 3.5 and s.mu == W.TWO_BAND_MU
+    s3 = fe.make_params(W.model_params(model=W.MODEL_THREE_BAND, mu=W.THREE_BAND_MU))
+    assert s3.model == 3 and list(s3.tb3) == list(W.THREE_BAND_T) and s3.band_mask == 7 and s3.cond_mult == 3.0
 
 
 def test_strerror_and_host_only_validation():
@@ -58,7 +60,7 @@ def test_strerror_and_host_only_validation():
     assert L.fe_create(C.byref(p), 8, float("nan"), C.byref(out)) == fe.FE_EINVAL
     bad = fe.make_params(W.model_params(U=0.0))
     assert L.fe_create(C.byref(bad), 8, 0.1, C.byref(out)) == fe.FE_EINVAL
-    bad = fe.make_params(dict(W.model_params(), model=3))
+    bad = fe.make_params(dict(W.model_params(), model=4))
     assert L.fe_create(C.byref(bad), 8, 0.1, C.byref(out)) == fe.FE_EINVAL
     assert b"model" in L.fe_strerror(fe.FE_EINVAL)
     assert L.fe_set_temperature(None, 0.1) == fe.FE_EINVAL

@@ -142,6 +142,48 @@ def test_coop_kernel_every_code_path(fe, oracle, flags):
                 parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=shape, flags=flags)
 
 
+# ---- three-band model: device Jacobi diagonalisation + per-q band tables + table-fed K1c ----
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("shape", [0, 1, 3])
+def test_three_band_parity(fe, oracle, shape, flags):
+    for w, temps in ((W.ragged3(), (0.002, 0.02, 2e-4)),
+                     (W.three_band(N=64, nq=3, nh=16, nd=40), (0.001,)),
+                     (W.three_band(N=48, nq=2, nh=70, nd=130, qdir="diag"), (0.003,))):
+        for T in temps:
+            parity(fe, oracle, w, T, shape=shape, flags=flags)
+
+
+def test_three_band_band_mask_const_mode_and_reuse(fe, oracle):
+    import torch
+    w = W.ragged3(seed=12, N=32, nq=2, nh=4, nd=9)
+    for mask in (1, 2, 4, 5):
+        w2 = W.Workload(w.name, dict(w.params, band_mask=mask, cond_mult=1.0), w.N, w.T, w.q, w.h, w.delta)
+        parity(fe, oracle, w2, 0.002)
+    w3 = W.Workload(w.name, dict(w.params, const_mode=1), w.N, w.T, w.q, w.h, w.delta)
+    parity(fe, oracle, w3, 0.002)
+    # one handle, several calls with different q lists (table 0 is cached, the q tables are rebuilt) and T
+    with fe.FreeEnergy(w.params, w.N, 0.002) as F:
+        for T, qs in ((0.002, w.q), (0.01, w.q[::-1].copy()), (0.002, np.vstack([w.q, w.q + 0.05, -w.q]))):
+            F.set_temperature(T)
+            om = F.omega_grid(qs, w.h, w.delta)
+            torch.cuda.synchronize()
+            ref = oracle.omega_grid(w.params, w.N, T, qs, w.h, w.delta)
+            assert max_rel(om.cpu().numpy(), ref) < RTOL
+        assert F.last_launch_info()["mode"] == fe.EVAL_COOP
+        with pytest.raises(fe.FeError):                      # per-thread kernels have no table path
+            F.set_eval_mode(fe.EVAL_DIRECT)
+            F.omega_grid(w.q, w.h, w.delta)
+
+
+def test_three_band_determinism_and_symmetry(fe):
+    w = W.three_band(N=96, nq=2, nh=8, nd=32)
+    a = run_gpu(fe, w, 0.001)[0]
+    b = run_gpu(fe, w, 0.001)[0]
+    assert np.array_equal(a, b)
+    wneg = W.Workload(w.name, w.params, w.N, w.T, w.q, w.h, -w.delta)
+    assert np.array_equal(run_gpu(fe, wneg, 0.001)[0], a)    # only Delta^2 enters
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
@@ -310,7 +352,10 @@ def test_full_size_configs_sampled_parity(fe, cfg, mode):
     import torch
     g = load_golden(cfg)
     w = W.config(cfg)
-    assert w.params == {k: (tuple(v) if isinstance(v, list) else v) for k, v in g["params"].items()}
+    # (the stored files predate the three-band field `tb3`, which configs 3-5 do not use)
+    assert {k: v for k, v in w.params.items() if k != "tb3"} == \
+        {k: (tuple(v) if isinstance(v, list) else v) for k, v in g["params"].items() if k != "tb3"}
+    assert not any(w.params["tb3"])
     for run in g["runs"]:
         T = run["T"]
         cols = run["columns"]
