@@ -304,3 +304,29 @@ int feo_argmin(const double* omega, const double* delta, int32_t ncol, int32_t n
     }
     return 0;
 }
+
+/* Outer loops of Algorithm 1: for a fixed field h the global ground state is
+ * the (q, Delta) pair of lowest Omega: "Omega_0 := +inf; for q: for Delta: if Omega < Omega_0 then save".
+ * omega is the grid of feo_omega_grid, index (iq*nh + ih)*nd + id.  ref_id >= 0: the value compared across q is the
+ * condensation energy Omega(q, h, Delta) - Omega(q, h, delta[ref_id]) (reading G17: for off-grid q the
+ * normal-state Omega itself depends on q at finite N); ref_id = -1: Omega itself, Algorithm 1 as printed.
+ * Strict '<' in loop order q, then Delta: the lowest (iq, id) wins among exact ties.                            */
+int feo_argmin_q(const double* omega, int32_t nq, int32_t nh, int32_t nd, int32_t ref_id,
+                 int32_t* iq_out, int32_t* id_out, double* value_out) {
+    if (!omega || nq < 1 || nh < 1 || nd < 1 || ref_id < -1 || ref_id >= nd) return -1;
+    for (int32_t ih = 0; ih < nh; ++ih) {
+        double best = INFINITY;
+        int32_t bq = 0, bd = 0;
+        for (int32_t iq = 0; iq < nq; ++iq) {
+            const double* col = omega + ((size_t)iq * nh + ih) * nd;
+            for (int32_t id = 0; id < nd; ++id) {
+                const double v = ref_id >= 0 ? col[id] - col[ref_id] : col[id];
+                if (v < best) { best = v; bq = iq; bd = id; }
+            }
+        }
+        if (iq_out) iq_out[ih] = bq;
+        if (id_out) id_out[ih] = bd;
+        if (value_out) value_out[ih] = best;
+    }
+    return 0;
+}

@@ -54,6 +54,8 @@ def lib():
         L.feo_omega_grid.restype = C.c_int
         L.feo_argmin.argtypes = [dp, dp, C.c_int32, C.c_int32, ip, dp, dp]
         L.feo_argmin.restype = C.c_int
+        L.feo_argmin_q.argtypes = [dp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, ip, ip, dp]
+        L.feo_argmin_q.restype = C.c_int
         _lib = L
     return _lib
 
@@ -161,3 +163,16 @@ def argmin(omega, delta):
         raise ValueError(f"feo_argmin failed: {rc}")
     shp = om.shape[:-1]
     return idx.reshape(shp), ds.reshape(shp), os_.reshape(shp)
+
+
+def argmin_q(omega, ref_id=-1):
+    """Per-h global minimum over (q, Delta) of Omega[iq, ih, id] (Algorithm 1 outer loops).
+    Returns (iq int32[nh], id int32[nh], value[nh]); value = Omega - Omega[..., ref_id] when ref_id >= 0."""
+    om = np.ascontiguousarray(omega, dtype=np.float64)
+    nq, nh, nd = om.shape
+    iq, idd, val = np.empty(nh, dtype=np.int32), np.empty(nh, dtype=np.int32), np.empty(nh)
+    ip = C.POINTER(C.c_int32)
+    rc = lib().feo_argmin_q(_dptr(om), nq, nh, nd, int(ref_id), iq.ctypes.data_as(ip), idd.ctypes.data_as(ip), _dptr(val))
+    if rc:
+        raise ValueError(f"feo_argmin_q failed: {rc}")
+    return iq, idd, val

@@ -479,6 +479,32 @@ def test_argmin_linear_search_lowest_index_on_ties(oracle):
     assert np.array_equal(os_, np.min(om, axis=-1))
 
 
+def test_argmin_q_outer_loop_of_algorithm_1(oracle):
+    """Algorithm 1 lines 1, 6-9 against numpy.argmin on the flattened (q, Delta) axis, with exact
+    ties (first occurrence in (iq, id) order wins) and with the condensation-energy reference (reading G17)."""
+    rng = np.random.default_rng(4)
+    om = rng.integers(-5, 5, size=(6, 7, 9)).astype(np.float64)        # many exact ties
+    iq, idd, val = oracle.argmin_q(om)
+    flat = om.transpose(1, 0, 2).reshape(7, -1)
+    assert np.array_equal(iq * 9 + idd, np.argmin(flat, axis=1))
+    assert np.array_equal(val, flat.min(axis=1))
+    om = rng.normal(size=(5, 4, 8))
+    iq, idd, val = oracle.argmin_q(om, ref_id=2)
+    ce = (om - om[:, :, 2:3]).transpose(1, 0, 2).reshape(4, -1)
+    assert np.array_equal(iq * 8 + idd, np.argmin(ce, axis=1)) and np.array_equal(val, ce.min(axis=1))
+    assert np.all(val <= 0.0)                                          # the reference point itself gives 0
+    with pytest.raises(ValueError):
+        oracle.argmin_q(om, ref_id=8)
+    # physics: on the interior-minimum grid the uniform state (q = 0) wins at h = 0 and is beaten or lost at high h
+    w = W.interior_minimum(N=32, U=5.0, T=0.005, nq=4, nh=4, nd=24)
+    g = oracle.omega_grid(w.params, w.N, w.T[0], w.q, w.h, w.delta)
+    iq, idd, val = oracle.argmin_q(g, ref_id=0)
+    assert iq[0] == 0 and idd[0] > 0 and val[0] < 0
+    cols_iq, cols_id, _ = oracle.argmin(g, w.delta)
+    for ih in range(w.nh):                                             # consistent with the per-(q, h) search
+        assert idd[ih] == cols_iq[iq[ih], ih]
+
+
 def test_grid_is_columns_in_q_h_delta_order(oracle):
     w = W.ragged(N=9, nq=2, nh=3, nd=5)
     om = oracle.omega_grid(w.params, w.N, w.T[0], w.q, w.h, w.delta)
