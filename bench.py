@@ -44,6 +44,7 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
     ("coop", (64, 128)): (2.382, 2.668, "ncu, profiles/r1d_ksum_coop_64x128_raw.csv (1.036 DADD + 1.060 DMUL + 0.286 DFMA)"),
+    ("coop", (64, 128), 3): (2.375, 2.656, "ncu, profiles/r1e_ksum_coop_3band_raw.csv (1.036 DADD + 1.059 DMUL + 0.281 DFMA)"),
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
     ("factored", (16, 4)): (4.20, 5.62, "ncu, profiles/r1c_ksum_factored_16x4_raw.csv"),
     ("direct", (4, 4)): (40.6, 61.3, "SASS count"),
@@ -52,7 +53,7 @@ KERNEL_COUNTS = {
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch from the ncu --set full capture in
 # profiles/ (a 1-q slice of the workload: 0.6 MB read, 95.5 MB written = the partial sums [ksplit][nh*nd]; the
 # launch timed here covers --q-per-step q-values and a different k-split, so this is context, not a bound: HBM is idle)
-KERNEL_TRAFFIC = {"coop": 96.1e6}
+KERNEL_TRAFFIC = {"coop": 96.1e6, ("coop", 3): 172.4e6}   # three-band: + 72 MB of band tables read
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
 PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
@@ -154,7 +155,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mode", default="coop", choices=["coop", "factored", "direct", "windowed"])
     ap.add_argument("--shape", type=int, default=0, help="block shape of the cooperative kernel (0 = auto)")
-    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--config", type=int, default=4, help="4 = BASELINE.json headline config; 6 = same shape, three-band model")
     ap.add_argument("--q-per-step", type=int, default=0, help="q-values per step (0 = the whole q list)")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--ref-deltas", type=int, default=64)
@@ -285,7 +286,8 @@ def main():
     info["block"] = 256
     if info["mode"] == fe.EVAL_COOP:
         info["block"] = next(c[4] for c in fe.coop_shapes() if (c[2], c[3]) == (info["th"], info["td"]))
-    counts = KERNEL_COUNTS.get((args.mode, (info["th"], info["td"])), (None, None, None))
+    tile_key = (args.mode, (info["th"], info["td"]))
+    counts = KERNEL_COUNTS.get(tile_key + (w.nbands,), KERNEL_COUNTS.get(tile_key, (None, None, None)))
     k_ms = sum(ksum_ms) / len(ksum_ms)
     dfma_rate, _ = fe.fp64_peak_probe()
     # Primary roofline = FP64-pipe lane-instructions/s: a DADD or DMUL occupies an FP64 lane for a cycle exactly like a
@@ -296,7 +298,7 @@ def main():
                 "peak": PEAK_DFMA_PER_S / 1e12,
                 "peak_source": "nominal: 148 SM x 64 FP64 lanes x 1.965 GHz (DESIGN.md section 6); MEASURED_PEAKS.json has no fp64 entry",
                 "peak_measured_dfma_probe": dfma_rate / 1e12, "avg_launch_ms": k_ms,
-                "band_evals_per_launch": band_evals, "traffic": KERNEL_TRAFFIC.get(args.mode),
+                "band_evals_per_launch": band_evals, "traffic": KERNEL_TRAFFIC.get((args.mode, w.nbands), KERNEL_TRAFFIC.get(args.mode)),
                 "kernel_share_of_step": k_ms * len(ksum_ms) / total_ms}
     if counts[0]:
         achieved = band_evals * counts[0] / (k_ms * 1e-3) / 1e12

@@ -119,6 +119,19 @@ int fe_argmin(fe_handle* h, const double* omega_dev, const double* delta,
               int32_t ncol, int32_t nd,
               int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev, void* cuda_stream);
 
+/* Global ground state per field h: minimum over (q, Delta) (outer loops of Algorithm 1, PAPER.md:133-153 lines 1, 6-9;
+ * "minimizing the free energy over the set of Delta and q").
+ *   omega_dev : DEVICE, nq*nh*nd doubles in the layout fe_omega_grid writes.
+ *   ref_id    : >= 0: the quantity compared across q is the condensation energy
+ *               Omega(q, h, Delta) - Omega(q, h, delta[ref_id]) (give the index of Delta = 0; for off-grid q the
+ *               normal-state Omega itself depends on q at finite N, reading G17);
+ *               -1: Omega itself, Algorithm 1 as printed.  Other values: FE_EINVAL.
+ *   iq_dev, id_dev (int32), value_dev (double) : DEVICE, nh each; any may be NULL.
+ * Lowest value wins; among exactly equal values the lowest iq, then the lowest Delta index.  NaN never wins.
+ * For the paper's per-band minimisation run one handle per band (band_mask).                        */
+int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, int32_t nd, int32_t ref_id,
+                int32_t* iq_dev, int32_t* id_dev, double* value_dev, void* cuda_stream);
+
 /* Host-buffer end-to-end path: copies the lists to the device, runs fe_omega_grid and fe_argmin,
  * copies results back and SYNCHRONISES the stream.  All pointers are HOST memory (pinned or pageable).
  *   omega_host : nq*nh*nd doubles or NULL (skip the Omega copy-back);

@@ -630,6 +630,17 @@ int fe_argmin(fe_handle* h, const double* omega_dev, const double* delta, int32_
   return argmin_impl(h, omega_dev, delta, ncol, nd, idx_dev, delta_star_dev, omega_star_dev, (cudaStream_t)cuda_stream);
 }
 
+int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, int32_t nd, int32_t ref_id,
+                int32_t* iq_dev, int32_t* id_dev, double* value_dev, void* cuda_stream) {
+  if (!h || !omega_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle or omega_dev is NULL"); return FE_EINVAL; }
+  if (nq < 1 || nh < 1 || nd < 1 || ref_id < -1 || ref_id >= nd) {
+    snprintf(g_errbuf, sizeof g_errbuf, "nq, nh, nd must be >= 1 and ref_id in [-1, nd)"); return FE_EINVAL; }
+  fe_argmin_q_kernel<<<nh, 256, 0, (cudaStream_t)cuda_stream>>>(nq, nh, nd, ref_id, omega_dev, iq_dev, id_dev, value_dev);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  return FE_OK;
+}
+
 int fe_scan_host(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                  const double* delta, int32_t nd, double* omega_host, int32_t* idx_host,
                  double* delta_star_host, double* omega_star_host, void* cuda_stream) {

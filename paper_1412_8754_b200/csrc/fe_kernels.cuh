@@ -643,6 +643,48 @@ __global__ void fe_argmin_kernel(int ncol, int nd, const double* __restrict__ om
 }
 
 // ---------------------------------------------------------------------------------------------------
+// K4: outer loops of Algorithm 1: per h the minimum over (q, Delta) of
+// Omega[iq][ih][id] (ref_id < 0) or of the condensation energy Omega[iq][ih][id] - Omega[iq][ih][ref_id].
+// One block per h; the flat index f = iq*nd + id is scanned in ascending order per thread, so the first occurrence
+// is kept, and the (value, f) lexicographic minimum is reduced over the block: lowest (iq, id) wins among ties.
+// NaN never wins; if nothing is below +inf the result is (0, 0, +inf).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fe_argmin_q_kernel(int nq, int nh, int nd, int ref_id,
+                                                          const double* __restrict__ omega, int32_t* __restrict__ iq_out,
+                                                          int32_t* __restrict__ id_out, double* __restrict__ val_out) {
+  const int ih = blockIdx.x;
+  const long long total = (long long)nq * nd;
+  double best = __longlong_as_double(0x7ff0000000000000LL);   // +inf
+  long long bf = 0x7fffffffffffffffLL;
+  for (long long f = threadIdx.x; f < total; f += blockDim.x) {
+    const int iq = (int)(f / nd), id = (int)(f - (long long)iq * nd);
+    const double* col = omega + ((size_t)iq * nh + ih) * nd;
+    const double v = ref_id >= 0 ? col[id] - col[ref_id] : col[id];
+    if (v < best) { best = v; bf = f; }
+  }
+  auto take = [&](double ov, long long of) {
+    if (ov < best || (ov == best && of < bf)) { best = ov; bf = of; }
+  };
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double ov = __shfl_down_sync(0xffffffffu, best, o);
+    const long long of = __shfl_down_sync(0xffffffffu, bf, o);
+    take(ov, of);
+  }
+  __shared__ double sv[8];
+  __shared__ long long sf[8];
+  if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = best; sf[threadIdx.x >> 5] = bf; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) take(sv[w], sf[w]);
+    if (bf == 0x7fffffffffffffffLL) bf = 0;
+    if (iq_out) iq_out[ih] = (int32_t)(bf / nd);
+    if (id_out) id_out[ih] = (int32_t)(bf % nd);
+    if (val_out) val_out[ih] = best;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 16 independent DFMA chains per thread, register-resident.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) fe_dfma_probe_kernel(int iters, double seed, double* __restrict__ sink) {

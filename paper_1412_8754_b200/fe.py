@@ -16,7 +16,7 @@ from . import build as _build
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP = 0, 1, 2, 3
 
-EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_scan_host",
+EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_scan_host",
            "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
@@ -229,6 +229,19 @@ class FreeEnergy:
                                C.c_void_p(idx.data_ptr()), C.c_void_p(ds.data_ptr()), C.c_void_p(os_.data_ptr()),
                                _stream(stream)))
         return idx, ds, os_
+
+    def argmin_q(self, omega, ref_id=-1, stream=None):
+        """Per-h global minimum over (q, Delta) of omega[iq, ih, id]: (iq int32, id int32, value) CUDA tensors [nh]."""
+        import torch
+        assert omega.is_cuda and omega.dtype == torch.float64 and omega.is_contiguous() and omega.dim() == 3
+        nq, nh, nd = omega.shape
+        iq = torch.empty(nh, dtype=torch.int32, device="cuda")
+        idd = torch.empty(nh, dtype=torch.int32, device="cuda")
+        val = torch.empty(nh, dtype=torch.float64, device="cuda")
+        _check(lib().fe_argmin_q(self._h, C.c_void_p(omega.data_ptr()), nq, nh, nd, int(ref_id),
+                                 C.c_void_p(iq.data_ptr()), C.c_void_p(idd.data_ptr()), C.c_void_p(val.data_ptr()),
+                                 _stream(stream)))
+        return iq, idd, val
 
     def scan_host(self, q, h, delta, want_omega=True, out=None, stream=None):
         """Host-buffer end-to-end path (fe_scan_host): numpy in, numpy out, synchronous.

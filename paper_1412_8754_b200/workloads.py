@@ -142,6 +142,10 @@ def config(i, seed=1):
                         _q_axis(np.linspace(0.0, 0.05 * pi, 16)),
                         np.linspace(0.1, 0.25, 16), np.linspace(0.0, 0.4, 1024),
                         "finite-size elimination, hoppings +-1%", extra=dict(seed=seed))
+    if i == 6:     # not in BASELINE.json: SURVEY.md 8(f-1), the shape of config 4 on the three-band model
+        b = three_band(N=1024, U=1.5, T=0.001, nq=32, nh=64, nd=512, qdir="diag")
+        b.name = "B3_fflo_N1024"
+        return b
     raise ValueError(f"no such config: {i}")
 
 

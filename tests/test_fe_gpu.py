@@ -184,6 +184,48 @@ def test_three_band_determinism_and_symmetry(fe):
     assert np.array_equal(run_gpu(fe, wneg, 0.001)[0], a)    # only Delta^2 enters
 
 
+# ---- outer loops of Algorithm 1: per-h minimum over (q, Delta) on the device ----
+def test_argmin_q_bit_exact_and_vs_oracle(fe, oracle):
+    import torch
+    rng = np.random.default_rng(6)
+    with fe.FreeEnergy(W.model_params(), 8, 0.01) as F:
+        # index work on given arrays: bit-exact against the oracle's linear search, exact ties, ragged sizes, NaN / inf
+        for shape in ((6, 7, 9), (1, 1, 1), (3, 2, 700), (300, 5, 3)):
+            om = rng.integers(-4, 4, size=shape).astype(np.float64)
+            if om.size > 20:
+                om.reshape(-1)[3] = np.nan
+                om.reshape(-1)[7] = np.inf
+            for ref in (-1, 0, shape[2] - 1):
+                iq, idd, val = F.argmin_q(torch.from_numpy(om).cuda(), ref_id=ref)
+                torch.cuda.synchronize()
+                r = oracle.argmin_q(om, ref_id=ref)
+                assert np.array_equal(iq.cpu().numpy(), r[0]) and np.array_equal(idd.cpu().numpy(), r[1])
+                assert np.array_equal(val.cpu().numpy(), r[2], equal_nan=True)
+        with pytest.raises(fe.FeError):
+            F.argmin_q(torch.zeros((2, 2, 2), dtype=torch.float64, device="cuda"), ref_id=2)
+    # end to end: device Omega -> device (q, Delta) minimum, against the oracle's grid and search
+    for w in (W.interior_minimum(N=48, U=5.0, T=0.004, nq=5, nh=6, nd=40), W.three_band(N=40, nq=4, nh=6, nd=30)):
+        T = w.T[0]
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            om = F.omega_grid(w.q, w.h, w.delta)
+            iq, idd, val = (x.cpu().numpy() for x in F.argmin_q(om, ref_id=0))
+            torch.cuda.synchronize()
+            omh = om.cpu().numpy()
+        r = oracle.argmin_q(omh, ref_id=0)                          # same Omega in: bit-exact out
+        assert np.array_equal(iq, r[0]) and np.array_equal(idd, r[1]) and np.array_equal(val, r[2])
+        ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        rq, rd, rv = oracle.argmin_q(ref, ref_id=0)
+        ce = ref - ref[:, :, :1]
+        scale = np.abs(ref).max()
+        for ih in range(w.nh):
+            flat = np.sort(ce[:, ih, :].reshape(-1))
+            if flat[1] - flat[0] > GAP * scale:                     # unique minimum: the index pair must agree
+                assert (iq[ih], idd[ih]) == (rq[ih], rd[ih])
+            else:                                                   # else any pair inside the band is valid
+                assert ce[iq[ih], ih, idd[ih]] - rv[ih] <= GAP * scale
+            assert abs(val[ih] - rv[ih]) <= 2 * RTOL * scale        # a difference of two Omega values
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
