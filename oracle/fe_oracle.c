@@ -330,3 +330,58 @@ int feo_argmin_q(const double* omega, int32_t nq, int32_t nh, int32_t nd, int32_
     }
     return 0;
 }
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Static Cooper-pair susceptibility, Appendix C, Eqs. C.2-C.3 at omega -> 0:
+ *
+ *   chi_{eps eps'}(q) = -(1/N) sum_k eta(-k-q)^2 [ f(-E_{eps k up}) - f(E_{eps',-k-q,down}) ] / ( -E_{eps k up} - E_{eps',-k-q,down} )
+ *
+ * N = number of lattice sites = number of k-points, f(x) = 1/(exp(x/T) + 1) the Fermi function, E_{eps k sigma}
+ * the band energies INCLUDING -(mu + sigma h) (Eq. 2), eta(k) = eta_scale cos kx cos ky
+ * (eta_scale = 4 is the paper's C.3 normalisation; reading G4).  The delta_{kl} of C.3 has been summed out.
+ * feo_pair_term is the summand's thermal factor  [f(-a) - f(b)] / (a + b)  evaluated literally in long double;
+ * at a + b = 0 exactly the quotient is 0/0 and its limit -f'(a) = 1 / (4 T cosh^2(a / 2T)) is used.
+ * chi_out[(iq*nb + eps)*nb + eps'], nb = number of bands.  Returns 0, -1 bad input.
+ * --------------------------------------------------------------------------------------------------------- */
+static long double feo_fermi_l(long double x, long double T) { return 1.0L / (expl(x / T) + 1.0L); }
+
+double feo_pair_term(double a, double b, double T) {
+    const long double al = a, bl = b, Tl = T;
+    const long double den = al + bl;
+    if (den == 0.0L) {
+        const long double c = coshl(al / (2.0L * Tl));
+        return (double)(1.0L / (4.0L * Tl * c * c));
+    }
+    return (double)((feo_fermi_l(-al, Tl) - feo_fermi_l(bl, Tl)) / den);
+}
+
+int feo_pair_susceptibility(const feo_params* p, int32_t N, double T, const double* q_xy, int32_t nq, double h,
+                            double* chi_out) {
+    if (!p || !q_xy || !chi_out || N < 1 || nq < 1 || !(T > 0.0)) return -1;
+    if (p->model != 1 && p->model != 2 && p->model != 3) return -1;
+    const int nb = feo_num_bands(p);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t iq = 0; iq < nq; ++iq) {
+        const double qx = q_xy[2 * iq], qy = q_xy[2 * iq + 1];
+        feo_acc A[9];
+        for (int i = 0; i < 9; ++i) { A[i].s = 0.0L; A[i].c = 0.0L; }
+        for (int32_t j = 0; j < N; ++j)
+            for (int32_t i = 0; i < N; ++i) {
+                const double kx = 2.0 * M_PI * (double)i / (double)N;
+                const double ky = 2.0 * M_PI * (double)j / (double)N;
+                double Ek[3], Ekq[3];
+                feo_band_energies(p, kx, ky, Ek);                    /* E_{eps}(k)     */
+                feo_band_energies(p, -kx - qx, -ky - qy, Ekq);       /* E_{eps'}(-k-q) */
+                const double eta = feo_eta(p, -kx - qx, -ky - qy);   /* eta(-k-q), C.2 */
+                for (int e = 0; e < nb; ++e)
+                    for (int f = 0; f < nb; ++f) {
+                        const double a = Ek[e] - p->mu - h;          /* E_{eps k up}          */
+                        const double b = Ekq[f] - p->mu + h;         /* E_{eps',-k-q,down}    */
+                        acc_add(&A[e * nb + f], (long double)(eta * eta) * (long double)feo_pair_term(a, b, T));
+                    }
+            }
+        for (int e = 0; e < nb * nb; ++e)
+            chi_out[(size_t)iq * nb * nb + e] = (double)((A[e].s + A[e].c) / ((long double)N * (long double)N));
+    }
+    return 0;
+}

@@ -54,6 +54,10 @@ def lib():
         L.feo_omega_grid.restype = C.c_int
         L.feo_argmin.argtypes = [dp, dp, C.c_int32, C.c_int32, ip, dp, dp]
         L.feo_argmin.restype = C.c_int
+        L.feo_pair_term.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.feo_pair_term.restype = C.c_double
+        L.feo_pair_susceptibility.argtypes = [pp, C.c_int32, C.c_double, dp, C.c_int32, C.c_double, dp]
+        L.feo_pair_susceptibility.restype = C.c_int
         L.feo_argmin_q.argtypes = [dp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, ip, ip, dp]
         L.feo_argmin_q.restype = C.c_int
         _lib = L
@@ -176,3 +180,20 @@ def argmin_q(omega, ref_id=-1):
     if rc:
         raise ValueError(f"feo_argmin_q failed: {rc}")
     return iq, idd, val
+
+
+def pair_term(a: float, b: float, T: float) -> float:
+    """[f(-a) - f(b)] / (a + b), the thermal factor of Eq. C.3 at omega = 0."""
+    return float(lib().feo_pair_term(a, b, T))
+
+
+def pair_susceptibility(p: dict, N: int, T: float, q, h: float) -> np.ndarray:
+    """chi[iq, eps, eps'] of Eqs. C.2-C.3 (static Cooper-pair susceptibility)."""
+    sp = _params(p)
+    q = np.ascontiguousarray(q, dtype=np.float64).reshape(-1, 2)
+    nb = {1: 1, 2: 2, 3: 3}[p["model"]]
+    out = np.empty((q.shape[0], nb, nb), dtype=np.float64)
+    rc = lib().feo_pair_susceptibility(C.byref(sp), N, T, _dptr(q), q.shape[0], float(h), _dptr(out))
+    if rc:
+        raise ValueError(f"feo_pair_susceptibility failed: {rc}")
+    return out
