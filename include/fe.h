@@ -132,6 +132,16 @@ int fe_argmin(fe_handle* h, const double* omega_dev, const double* delta,
 int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, int32_t nd, int32_t ref_id,
                 int32_t* iq_dev, int32_t* id_dev, double* value_dev, void* cuda_stream);
 
+/* Static Cooper-pair susceptibility of Appendix C, Eqs. C.2-C.3 at omega -> 0, at the handle's
+ * temperature and one Zeeman field hz:
+ *   chi_{e f}(q) = (1/N^2) sum_k eta(-k-q)^2 [f(-E_{e,k,up}) - f(E_{f,-k-q,down})] / (E_{e,k,up} + E_{f,-k-q,down}),
+ * f = Fermi function, E_{e,k,sigma} = E_e(k) - mu - sigma hz, eta from form_factor / eta_scale (4.0 = the paper's C.3).
+ *   q_xy    : HOST, nq pairs (qx, qy), any real vectors (copied before return).
+ *   chi_dev : DEVICE, nq * nb * nb doubles, index (iq*nb + e)*nb + f, nb = number of bands (band_mask is ignored).
+ * Asynchronous on cuda_stream; deterministic.  With fe_enable_timing the k-sum kernel of this call is the one
+ * fe_get_timing reports (its second value is then the number of (k, q, e, f) pair terms).               */
+int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream);
+
 /* Host-buffer end-to-end path: copies the lists to the device, runs fe_omega_grid and fe_argmin,
  * copies results back and SYNCHRONISES the stream.  All pointers are HOST memory (pinned or pageable).
  *   omega_host : nq*nh*nd doubles or NULL (skip the Omega copy-back);

@@ -340,7 +340,7 @@ int feo_argmin_q(const double* omega, int32_t nq, int32_t nh, int32_t nd, int32_
  * the band energies INCLUDING -(mu + sigma h) (Eq. 2), eta(k) = eta_scale cos kx cos ky
  * (eta_scale = 4 is the paper's C.3 normalisation; reading G4).  The delta_{kl} of C.3 has been summed out.
  * feo_pair_term is the summand's thermal factor  [f(-a) - f(b)] / (a + b)  evaluated literally in long double;
- * at a + b = 0 exactly the quotient is 0/0 and its limit -f'(a) = 1 / (4 T cosh^2(a / 2T)) is used.
+ * at a + b -> 0 the quotient is 0/0 and its limit -f'((a-b)/2) = 1 / (4 T cosh^2((a-b) / 4T)) is used.
  * chi_out[(iq*nb + eps)*nb + eps'], nb = number of bands.  Returns 0, -1 bad input.
  * --------------------------------------------------------------------------------------------------------- */
 static long double feo_fermi_l(long double x, long double T) { return 1.0L / (expl(x / T) + 1.0L); }
@@ -348,8 +348,11 @@ static long double feo_fermi_l(long double x, long double T) { return 1.0L / (ex
 double feo_pair_term(double a, double b, double T) {
     const long double al = a, bl = b, Tl = T;
     const long double den = al + bl;
-    if (den == 0.0L) {
-        const long double c = coshl(al / (2.0L * Tl));
+    /* Removable singularity of C.3 (reading G19): with a = m + e, b = -m + e the quotient is the central
+     * difference [f(-m-e) - f(-m+e)] / (2e) = -f'(m) (1 + O((e/T)^2)); for |a + b| <= 1e-6 T the literal quotient
+     * would lose its digits to cancellation (it is 0/0 at e = 0) while the limit is exact to 1e-13. */
+    if (fabsl(den) <= 1e-6L * Tl) {
+        const long double c = coshl((al - bl) / (4.0L * Tl));
         return (double)(1.0L / (4.0L * Tl * c * c));
     }
     return (double)((feo_fermi_l(-al, Tl) - feo_fermi_l(bl, Tl)) / den);

@@ -11,6 +11,7 @@
 #define FE_PLAIN_KERNELS
 #include "fe_kernels.cuh"
 #include "fe_bands3.cuh"
+#include "fe_chi.cuh"
 #include "fe_launch.h"
 
 namespace {
@@ -636,6 +637,75 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
   if (nq < 1 || nh < 1 || nd < 1 || ref_id < -1 || ref_id >= nd) {
     snprintf(g_errbuf, sizeof g_errbuf, "nq, nh, nd must be >= 1 and ref_id in [-1, nd)"); return FE_EINVAL; }
   fe_argmin_q_kernel<<<nh, 256, 0, (cudaStream_t)cuda_stream>>>(nq, nh, nd, ref_id, omega_dev, iq_dev, id_dev, value_dev);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  return FE_OK;
+}
+
+int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
+  if (!h || !q_xy || !chi_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle, q_xy or chi_dev is NULL"); return FE_EINVAL; }
+  if (nq < 1 || nq > 65535 || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, 65535], hz finite"); return FE_EINVAL; }
+  for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int N = h->N, nb = h->nb, nbb = nb * nb;
+  double *hs, *ds; StageSlot* slot;
+  int rc = stage_lists(h, (size_t)2 * nq, st, &hs, &ds, &slot);
+  if (rc) return rc;
+  for (int i = 0; i < 2 * nq; ++i) hs[i] = -q_xy[i];          // tables of k - (-q) = k + q; E, eta even: = -k - q
+  FE_CUDA(cudaMemcpyAsync(ds, hs, (size_t)2 * nq * sizeof(double), cudaMemcpyHostToDevice, st));
+  FE_CUDA(cudaEventRecord(slot->ev, st));
+  slot->pending = true;
+  const unsigned long long nk = (unsigned long long)N * N;
+  long long nchunk = ((long long)h->sm_count * 16 + nq - 1) / nq;                  // >= 16 blocks per SM in total
+  const long long max_chunk = (long long)((nk + 4 * kThreads - 1) / (4 * kThreads));  // >= 4 k-points per thread
+  if (nchunk > max_chunk) nchunk = max_chunk;
+  if (nchunk < 1) nchunk = 1;
+  if (nchunk > 65535) nchunk = 65535;
+  unsigned long long kc = (nk + nchunk - 1) / nchunk;
+  kc = (kc + kThreads - 1) / kThreads * kThreads;
+  nchunk = (long long)((nk + kc - 1) / kc);
+  if ((rc = ensure(h->d_coltab, h->coltab_cap, (size_t)nq * N))) return rc;
+  if ((rc = ensure(h->d_rowtab, h->rowtab_cap, (size_t)nq * N))) return rc;
+  if ((rc = ensure(h->d_partial, h->partial_cap, (size_t)nchunk * nq * nbb))) return rc;
+  if (nb == 3) {
+    const size_t need = (size_t)(1 + nq) * 3 * N * N;
+    if (need > h->etab_cap || !h->d_etab) h->etab_base_valid = false;
+    if ((rc = ensure(h->d_etab, h->etab_cap, need))) return rc;
+  }
+  fe_trig_kernel<<<(N * nq + 255) / 256, 256, 0, st>>>(N, nq, ds, h->d_coltab, h->d_rowtab);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  if (nb == 3) {
+    Band3Consts bc;
+    for (int i = 0; i < 12; ++i) bc.t[i] = h->p.tb3[i];
+    bc.e0 = h->p.tb3[12];
+    const int y0 = h->etab_base_valid ? 1 : 0;
+    dim3 g((unsigned)((nk + 255) / 256), (unsigned)(1 + nq - y0));
+    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, h->d_etab);
+    FE_CUDA(cudaGetLastError());
+    h->etab_base_valid = true;
+    h->launches++;
+  }
+  const ModelConsts mc = make_consts(h->p);
+  dim3 grid((unsigned)nchunk, (unsigned)nq);
+  if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
+  const int form = h->p.form_factor;
+#define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, h->d_partial)
+  if (nb == 1) { if (form == 0) FE_CHI(1, 0); else FE_CHI(1, 1); }
+  else if (nb == 2) { if (form == 0) FE_CHI(2, 0); else FE_CHI(2, 1); }
+  else { if (form == 0) FE_CHI(3, 0); else FE_CHI(3, 1); }
+#undef FE_CHI
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  if (h->timing) {
+    FE_CUDA(cudaEventRecord(h->ev1, st));
+    h->timing_valid = true;
+    h->last_band_evals = (double)nk * nq * nbb;
+  }
+  h->last_info[0] = nb; h->last_info[1] = nb; h->last_info[2] = (int32_t)nchunk; h->last_info[3] = (int32_t)(nchunk * nq);
+  h->last_info[4] = -1; h->last_info[5] = (int32_t)(kc < 2147483647ULL ? kc : 2147483647ULL);
+  const int nout = nq * nbb;
+  fe_chi_finish_kernel<<<(nout + 255) / 256, 256, 0, st>>>(nout, (int)nchunk, 1.0 / ((double)N * (double)N), h->d_partial, chi_dev);
   FE_CUDA(cudaGetLastError());
   h->launches++;
   return FE_OK;

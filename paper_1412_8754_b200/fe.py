@@ -16,7 +16,7 @@ from . import build as _build
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP = 0, 1, 2, 3
 
-EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_scan_host",
+EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility", "fe_scan_host",
            "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
@@ -60,6 +60,8 @@ def lib():
     L.fe_set_eval_mode.argtypes = [vp, C.c_int32]
     L.fe_omega_grid.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, vp, vp]
     L.fe_argmin.argtypes = [vp, vp, dp, C.c_int32, C.c_int32, vp, vp, vp, vp]
+    L.fe_argmin_q.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, vp]
+    L.fe_pair_susceptibility.argtypes = [vp, dp, C.c_int32, C.c_double, vp, vp]
     L.fe_scan_host.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, vp, vp, vp, vp, vp]
     L.fe_enable_timing.argtypes = [vp, C.c_int32]
     L.fe_get_timing.argtypes = [vp, C.POINTER(C.c_float), dp]
@@ -148,7 +150,7 @@ class FreeEnergy:
         self._h = C.c_void_p()
         self._params = make_params(params)
         self.N, self.T = int(N), float(T)
-        self.nbands = 1 if params["model"] == 1 else 2
+        self.nbands = {1: 1, 2: 2, 3: 3}[int(params["model"])]
         _check(lib().fe_create(C.byref(self._params), self.N, self.T, C.byref(self._h)))
 
     def close(self):
@@ -242,6 +244,18 @@ class FreeEnergy:
                                  C.c_void_p(iq.data_ptr()), C.c_void_p(idd.data_ptr()), C.c_void_p(val.data_ptr()),
                                  _stream(stream)))
         return iq, idd, val
+
+    def pair_susceptibility(self, q, hz, out=None, stream=None):
+        """chi[iq, e, f] (Appendix C) as a CUDA torch tensor (float64).  Asynchronous on `stream`."""
+        import torch
+        q = _f64(q).reshape(-1, 2)
+        nb = self.nbands
+        if out is None:
+            out = torch.empty((q.shape[0], nb, nb), dtype=torch.float64, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == q.shape[0] * nb * nb
+        _check(lib().fe_pair_susceptibility(self._h, _dptr(q), q.shape[0], C.c_double(float(hz)),
+                                            C.c_void_p(out.data_ptr()), _stream(stream)))
+        return out
 
     def scan_host(self, q, h, delta, want_omega=True, out=None, stream=None):
         """Host-buffer end-to-end path (fe_scan_host): numpy in, numpy out, synchronous.

@@ -179,6 +179,24 @@ def ragged3(seed=11, N=37, nq=3, nh=5, nd=19):
                     np.sort(rng.uniform(-0.02, 0.16, size=nd)), "ragged sizes, three bands")
 
 
+def chi_map(model=MODEL_TWO_BAND, N=256, nside=16, T=0.001, h=0.025, on_grid=True):
+    """q map of the static Cooper-pair susceptibility (Appendix C; Fig. C.6 is at h = 0.025 eV,
+    k_B T ~ 0, eta = 4 cos kx cos ky): nside x nside q-points over the quadrant [0, pi]^2, snapped to the k-grid
+    when on_grid.  Returned as a Workload whose h list holds the single field and whose Delta list is unused."""
+    v = np.linspace(0.0, math.pi, nside)
+    if on_grid:
+        v = 2.0 * math.pi * np.round(v * N / (2.0 * math.pi)) / N
+    q = np.stack(np.meshgrid(v, v, indexing="ij"), axis=-1).reshape(-1, 2)
+    if model == MODEL_THREE_BAND:
+        p = model_params(model=MODEL_THREE_BAND, mu=THREE_BAND_MU, U=1.5, eta_scale=4.0)
+    elif model == MODEL_TWO_BAND:
+        p = model_params(eta_scale=4.0)
+    else:
+        p = model_params(model=MODEL_ONE_BAND, form_factor=FORM_S, t=(1.0,), mu=-0.3, U=2.0)
+    return Workload(f"chi_m{model}_N{N}_q{nside}x{nside}", p, N, (T,), q, np.array([h]), np.array([0.0]),
+                    "pair-susceptibility q map")
+
+
 def ragged(seed=7, N=45, nq=3, nh=5, nd=37, model=MODEL_TWO_BAND):
     """Deliberately awkward sizes: odd N, list lengths that divide no tile, off-grid q, negative h/Delta."""
     rng = np.random.default_rng(seed)

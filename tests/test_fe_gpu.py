@@ -226,6 +226,51 @@ def test_argmin_q_bit_exact_and_vs_oracle(fe, oracle):
             assert abs(val[ih] - rv[ih]) <= 2 * RTOL * scale        # a difference of two Omega values
 
 
+# ---- static Cooper-pair susceptibility ----
+@pytest.mark.parametrize("model", [1, 2, 3])
+def test_pair_susceptibility_parity(fe, oracle, model):
+    import torch
+    rng = np.random.default_rng(model)
+    for N, T, h, on_grid in ((37, 0.004, 0.025, False), (48, 0.001, 0.025, True), (20, 0.3, -0.1, False), (64, 1e-4, 0.0, True)):
+        w = W.chi_map(model=model, N=N, nside=5, T=T, h=h, on_grid=on_grid)
+        q = w.q if on_grid else w.q + rng.uniform(-0.3, 0.3, size=w.q.shape)
+        for form in (W.FORM_S, W.FORM_SPM):
+            p = dict(w.params, form_factor=form)
+            with fe.FreeEnergy(p, N, T) as F:
+                chi = F.pair_susceptibility(q, h)
+                chi2 = F.pair_susceptibility(q, h)
+                torch.cuda.synchronize()
+            ref = oracle.pair_susceptibility(p, N, T, q, h)
+            assert torch.equal(chi, chi2)                                  # deterministic
+            err = np.max(np.abs(chi.cpu().numpy() - ref) / np.abs(ref).max(axis=(1, 2), keepdims=True))
+            # conditioning (chi): near the Fermi surface g = tanh(a/2T)/(2a) varies on the
+            # scale T, so the <= 1 ulp rounding of E_k (|E| <= W) is magnified by W/T before any arithmetic of ours
+            Wband = {1: 4.0, 2: 8.0, 3: 2.0}[model]
+            tol = RTOL + 0.5 * np.finfo(float).eps * Wband / T
+            assert err < tol, f"chi model {model} N={N} T={T} form={form}: {err:.3e} (tol {tol:.1e})"
+
+
+def test_pair_susceptibility_degenerate_and_errors(fe, oracle):
+    import torch
+    # exactly cancelling pairs a + b = 0 (q = 0, h = 0: a = b, and mu on a band energy), N = 1, one q
+    p = W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(1.0,), mu=0.0, U=2.0)
+    for N, T in ((1, 0.1), (4, 0.05), (8, 1e-3)):
+        with fe.FreeEnergy(p, N, T) as F:
+            chi = F.pair_susceptibility([(0.0, 0.0), (np.pi, np.pi)], 0.0).cpu().numpy()
+        ref = oracle.pair_susceptibility(p, N, T, [(0.0, 0.0), (np.pi, np.pi)], 0.0)
+        assert max_rel(chi, ref) < RTOL
+    with fe.FreeEnergy(p, 8, 0.1) as F:
+        with pytest.raises(fe.FeError):
+            F.pair_susceptibility([(np.nan, 0.0)], 0.0)
+        with pytest.raises(fe.FeError):
+            F.pair_susceptibility([(0.0, 0.0)], np.inf)
+        # the handle still serves the free-energy path afterwards (shared scratch)
+        w = W.config(1)
+        om = F.omega_grid(w.q, w.h, w.delta)
+        torch.cuda.synchronize()
+        assert torch.isfinite(om).all()
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""

@@ -37,6 +37,10 @@ def test_pair_term_is_the_lehmann_sum(oracle):
         lim = 1.0 / (4 * T * math.cosh(a / (2 * T)) ** 2)
         assert abs(oracle.pair_term(a, -a, T) - lim) < 1e-14 * max(lim, 1)
         assert abs(oracle.pair_term(a, -a + 1e-7, T) - lim) < 1e-5 * max(lim, 1)
+        # rounding-noise-sized sums (perfect nesting E(k+Q) = -E(k) in floating point) stay on the limit
+        for e in (1e-16, -3e-17, 1e-12, 0.9e-6 * T, 1.1e-6 * T, 1e-5 * T):
+            mid = 1.0 / (4 * T * math.cosh((2 * a - e) / (4 * T)) ** 2)          # -f' at the midpoint (a - b)/2
+            assert abs(oracle.pair_term(a, -a + e, T) - mid) < 1e-9 * mid, e
     # deep in the Fermi sea / far above it and huge |x|/T: no overflow, 1/(|a|+|b|) for same-sign pairs
     assert abs(oracle.pair_term(3.0, 2.0, 1e-4) - 1 / 5.0) < 1e-15
     assert abs(oracle.pair_term(-3.0, -2.0, 1e-4) - 1 / 5.0) < 1e-15
