@@ -24,9 +24,11 @@ struct ChiSide { double x, ax, u, opu, th; };   // energy, |energy|, exp(-|x|/T)
 __device__ __forceinline__ ChiSide chi_side(double x, double neg_beta) {
   ChiSide s;
   s.x = x; s.ax = fabs(x);
-  s.u = exp(s.ax * neg_beta);
-  s.opu = 1.0 + s.u;
-  s.th = (1.0 - s.u) / s.opu;
+  const double t = s.ax * neg_beta;            // -|x|/T <= 0
+  s.u = exp(t);                                // keeps its relative accuracy when tiny (w in the blocked pairs)
+  const double em = t > -0.6931 ? expm1(t) : s.u - 1.0;   // u - 1 without cancellation for |x| << T (states on
+  s.opu = 1.0 + s.u;                                      // the Fermi surface): tanh(|x|/2T) = (1-u)/(1+u)
+  s.th = -em / s.opu;
   return s;
 }
 
