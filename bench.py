@@ -147,6 +147,87 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+# FP64-pipe instructions per (k, q) point of the susceptibility kernel (all nb^2 band pairs), ncu (profiles/r1f_*)
+CHI_COUNTS = {(2,): (238.0, "ncu, profiles/r1f_chi_2band_raw.csv (153.0 DFMA + 43.4 DADD + 41.5 DMUL per (k, q) point, 4 band pairs)")}
+
+
+def run_chi(args):
+    """q map of the static Cooper-pair susceptibility (Appendix C).  One step = fe_pair_susceptibility
+    over the whole q list (K0 trig, [KB bands], K-chi k-sum, finish).  value = (k, q) points per second."""
+    import torch
+    from paper_1412_8754_b200 import fe
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: no CUDA device visible (there is no CPU fallback)")
+    torch.cuda.set_device(0)
+    w = W.chi_map(model=args.chi_model, N=args.chi_N, nside=args.chi_nside, T=0.001, h=0.025)
+    F = fe.FreeEnergy(w.params, w.N, w.T[0])
+    F.enable_timing(True)
+    stream = torch.cuda.current_stream()
+    nb = w.nbands
+    chi = torch.empty((w.nq, nb, nb), dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+    hz = float(w.h[0])
+    for _ in range(args.warmup):
+        F.pair_susceptibility(w.q, hz, out=chi, stream=stream)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    l0 = F.launch_count()
+    step_ms, k_ms = [], []
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        F.pair_susceptibility(w.q, hz, out=chi, stream=stream)
+        e1.record(stream)
+        e1.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        k_ms.append(F.last_ksum()[0])
+    torch.cuda.synchronize()
+    launches = F.launch_count() - l0
+    clocks = sampler.stop()
+    points = w.N * w.N * w.nq
+    value = points * args.steps / (sum(step_ms) * 1e-3)
+    host = torch.empty((w.nq, nb, nb), dtype=torch.float64).pin_memory()
+    hq = torch.from_numpy(w.q.copy()).pin_memory().numpy()
+    t0 = time.perf_counter()
+    for _ in range(2):
+        F.pair_susceptibility(hq, hz, out=chi, stream=stream)
+        host.copy_(chi, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e = points * 2 / (time.perf_counter() - t0)
+    kms = sum(k_ms) / len(k_ms)
+    dfma_rate, _ = fe.fp64_peak_probe()
+    cnt = CHI_COUNTS.get((args.chi_model,))
+    roofline = {"bound": "alu", "kernel": f"fe_chi_kernel<{nb}, {w.params['form_factor']}>", "unit": "Tinst/s (FP64-pipe thread-instructions)",
+                "peak": PEAK_DFMA_PER_S / 1e12, "peak_measured_dfma_probe": dfma_rate / 1e12, "avg_launch_ms": kms,
+                "kernel_share_of_step": kms * len(k_ms) / sum(step_ms), "traffic": None,
+                "achieved": None, "frac": None}
+    if cnt:
+        ach = points * cnt[0] / (kms * 1e-3) / 1e12
+        roofline.update({"achieved": ach, "frac": ach / (PEAK_DFMA_PER_S / 1e12), "fp64_inst_per_kq_point": cnt[0],
+                         "counts_source": cnt[1]})
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import fe_oracle as O
+        nsamp = max(1, min(w.nq, O.num_threads()))
+        t0 = time.perf_counter()
+        ref = O.pair_susceptibility(w.params, w.N, w.T[0], w.q[:nsamp], hz)
+        dt = time.perf_counter() - t0
+        err = float(np.max(np.abs(chi[:nsamp].cpu().numpy() - ref) / np.abs(ref).max()))
+        cpu = {"value": w.N * w.N * nsamp / dt, "unit": "(k, q) points/s", "cores": O.num_threads(), "kind": "oracle",
+               "seconds": dt, "sample": f"first {nsamp} of {w.nq} q-points, full {w.N}x{w.N} k-sum", "max_rel_err_vs_gpu": err}
+    line = {"metric": "pair-susceptibility (k, q) point evaluations/s (all band pairs, fp64)", "value": value,
+            "unit": "(k, q) points/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": sum(step_ms) / len(step_ms), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "nq": w.nq, "bands": nb, "T": w.T[0], "h": hz,
+                       "pair_terms_per_step": points * nb * nb, "l2": "flushed between timed steps (256 MB memset)"},
+            "e2e": {"value": e2e, "unit": "(k, q) points/s", "h2d_bytes_per_step": 16 * w.nq, "d2h_bytes_per_step": 8 * w.nq * nb * nb},
+            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -161,7 +242,14 @@ def main():
     ap.add_argument("--ref-deltas", type=int, default=64)
     ap.add_argument("--cpu-baseline-deltas", type=int, default=256)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="omega", choices=["omega", "chi"],
+                    help="omega = the free-energy scan (BASELINE.json metric); chi = pair-susceptibility q map (SURVEY 8f-4)")
+    ap.add_argument("--chi-model", type=int, default=2)
+    ap.add_argument("--chi-N", type=int, default=1024)
+    ap.add_argument("--chi-nside", type=int, default=48)
     args = ap.parse_args()
+    if args.workload == "chi":
+        return run_chi(args)
 
     w = W.config(args.config)
     if args.impl == "reference":
