@@ -234,7 +234,8 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="coop", choices=["coop", "factored", "direct", "windowed"])
+    ap.add_argument("--mode", default="coop_eo", choices=["coop_eo", "coop", "factored", "direct", "windowed"],
+                    help="coop_eo = library default (early-out); coop = dense variant (every pair multiplied out)")
     ap.add_argument("--shape", type=int, default=0, help="block shape of the cooperative kernel (0 = auto)")
     ap.add_argument("--config", type=int, default=4, help="4 = BASELINE.json headline config; 6 = same shape, three-band model")
     ap.add_argument("--q-per-step", type=int, default=0, help="q-values per step (0 = the whole q list)")
@@ -277,7 +278,7 @@ def main():
     else:
         q_all = w.q
     temps = list(w.T)
-    mode = {"coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
+    mode = {"coop_eo": fe.EVAL_COOP_EO, "coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
             "windowed": fe.EVAL_WINDOWED}[args.mode]
 
     F = fe.FreeEnergy(w.params, w.N, temps[0])
@@ -372,7 +373,7 @@ def main():
     # ---- roofline of the dominant kernel (K1 k-sum) ----
     info = F.last_launch_info()
     info["block"] = 256
-    if info["mode"] == fe.EVAL_COOP:
+    if info["mode"] in (fe.EVAL_COOP, fe.EVAL_COOP_EO):
         info["block"] = next(c[4] for c in fe.coop_shapes() if (c[2], c[3]) == (info["th"], info["td"]))
     tile_key = (args.mode, (info["th"], info["td"]))
     counts = KERNEL_COUNTS.get(tile_key + (w.nbands,), KERNEL_COUNTS.get(tile_key, (None, None, None)))

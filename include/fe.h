@@ -47,12 +47,16 @@ extern "C" {
                                  the 3x3 complex-Hermitian T_k is diagonalised numerically on the device and the
                                  eigenvalues are stored in per-q tables in HBM, as the paper proposes for more than two
                                  bands; band e = e-th eigenvalue in ascending order.
-                                 FE_EVAL_COOP only.                                                                */
+                                 FE_EVAL_COOP / FE_EVAL_COOP_EO only.                                              */
 #define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
 #define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
 
-/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all four compute the same sums ----
- * COOP    : default.  The factored form below, block-cooperative: a thread block owns one (h, Delta) block tile and
+/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all five compute the same sums ----
+ * COOP_EO : default.  COOP with a block-uniform early-out: a (k, band) slot whose 2cosh(R_j/T) exceeds 2cosh(|d_i|/T)
+ *           by more than 2^58 over the whole block tile contributes T ln Z_ij = R_j (exact to fp64), so it is summed
+ *           per Delta_j without exponentials or pair products; the other slots are compacted and run through COOP's
+ *           dense pipeline.  Same results to ~1e-15 relative; several times fewer FP64 instructions at low T.
+ * COOP    : the dense variant (every pair of every slot is multiplied out).  The factored form below, block-cooperative: a thread block owns one (h, Delta) block tile and
  *           a chunk of k-points; the WD + WH exponentials per (k, band) are computed once per block and shared
  *           through shared memory; every thread keeps a TH x TD register tile of running products over all k of
  *           the chunk (no cross-thread reduction).  Falls back to FACTORED when the grid is much smaller than a
@@ -68,6 +72,7 @@ extern "C" {
 #define FE_EVAL_DIRECT   1
 #define FE_EVAL_WINDOWED 2
 #define FE_EVAL_COOP     3
+#define FE_EVAL_COOP_EO  4
 
 typedef struct fe_handle fe_handle; /* opaque; owns device scratch (trig tables, partial sums, staging) */
 
@@ -93,7 +98,7 @@ int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** ou
 /* Change T (> 0, finite) for subsequent calls (config 4 scans two temperatures).  Host-only, cheap. */
 int fe_set_temperature(fe_handle* h, double T);
 
-/* Select FE_EVAL_COOP (default), FE_EVAL_FACTORED, FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
+/* Select FE_EVAL_COOP_EO (default), FE_EVAL_COOP, FE_EVAL_FACTORED, FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
 int fe_set_eval_mode(fe_handle* h, int32_t mode);
 
 /* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,

@@ -55,7 +55,7 @@ struct fe_handle {
   fe_model_params p;
   int32_t N = 0;
   double T = 0;
-  int32_t mode = FE_EVAL_COOP;
+  int32_t mode = FE_EVAL_COOP_EO;
   int32_t tile = 0;            // 0 = auto, else 1 + index
   int32_t target_blocks = 0;   // 0 = auto
   int32_t debug_flags = 0;
@@ -286,8 +286,10 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
   int mode = h->mode;
   int cshape = 0;
+  const bool early_out = mode == FE_EVAL_COOP_EO;
+  if (early_out) mode = FE_EVAL_COOP;                       // same kernel, CoopParams.early_out = 1
   if (h->nb == 3 && mode != FE_EVAL_COOP) {
-    snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND supports FE_EVAL_COOP only"); return FE_EINVAL; }
+    snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND supports FE_EVAL_COOP / FE_EVAL_COOP_EO only"); return FE_EINVAL; }
   if (mode == FE_EVAL_COOP) {
     cshape = choose_coop_shape(h, nh, nd);
     if (h->nb == 3 && kCoopShapes[cshape].lh != 4) {
@@ -305,7 +307,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   }
   const bool coop = mode == FE_EVAL_COOP;
   // ---- stage lists: [q (2nq) | h (nh) | delta^2 (nd)] ----
-  const int tile = choose_tile_mode(mode == h->mode ? h->tile : 0, mode, nh, nd);
+  const int tile = choose_tile_mode((mode == h->mode || (early_out && mode == FE_EVAL_COOP)) ? h->tile : 0, mode, nh, nd);
   const int TH = kTiles[tile].th, TD = kTiles[tile].td;
   const int ntile_h = (nh + TH - 1) / TH;
   const int hstride = htile_stride(TH);
@@ -404,6 +406,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     CP.N = N; CP.nq = nq; CP.nh = nh; CP.nd = nd;
     CP.ntile_h = (nh + wh - 1) / wh; CP.ntile_d = (nd + wd - 1) / wd;
     CP.debug_flags = h->debug_flags;
+    CP.early_out = early_out ? 1 : 0;
     CP.nk = (unsigned long long)N * (unsigned long long)N;
     const long long ctiles = (long long)nq * CP.ntile_h * CP.ntile_d;
     const long long wave = (long long)h->sm_count * cs.minb;
@@ -482,7 +485,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     h->launches++;
   }
   h->last_info[0] = TH; h->last_info[1] = TD; h->last_info[2] = P.ksplit; h->last_info[3] = (int32_t)grid_ll;
-  h->last_info[4] = mode; h->last_info[5] = P.rows_per_chunk;
+  h->last_info[4] = (coop && early_out) ? FE_EVAL_COOP_EO : mode; h->last_info[5] = P.rows_per_chunk;
   if (coop) {
     const CoopShape& cs = kCoopShapes[cshape];
     h->last_info[0] = cs.th * cs.lh; h->last_info[1] = cs.td * cs.nw * (32 / cs.lh);     // block tile WH x WD
@@ -572,7 +575,8 @@ int fe_set_temperature(fe_handle* h, double T) {
 
 int fe_set_eval_mode(fe_handle* h, int32_t mode) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
-  if (mode != FE_EVAL_FACTORED && mode != FE_EVAL_DIRECT && mode != FE_EVAL_WINDOWED && mode != FE_EVAL_COOP) {
+  if (mode != FE_EVAL_FACTORED && mode != FE_EVAL_DIRECT && mode != FE_EVAL_WINDOWED && mode != FE_EVAL_COOP &&
+      mode != FE_EVAL_COOP_EO) {
     snprintf(g_errbuf, sizeof g_errbuf, "unknown eval mode %d", mode); return FE_EINVAL; }
   h->mode = mode;
   return FE_OK;

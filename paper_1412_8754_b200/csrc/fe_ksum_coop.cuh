@@ -42,6 +42,7 @@ struct CoopParams {
   int32_t N, nq, nh, nd;
   int32_t ntile_h, ntile_d, ksplit;
   int32_t debug_flags;                 // bit 0: every slot takes the robust path (tests)
+  int32_t early_out;                   // 1: A-dominated slots bypass the pair products (FE_EVAL_COOP_EO)
   unsigned long long kc;               // k-points per chunk (multiple of the block size)
   unsigned long long nk;               // N*N
   const double4* coltab;               // [nq][N] {cos kx, sin kx, cos(kx-qx), sin(kx-qx)}
@@ -59,6 +60,9 @@ struct __align__(16) CoopHdr {         // one per (k, band) slot
   int flags;                           // bit 0 skip, bit 1 robust, bits 8.. = drift step
 };
 constexpr int kCoopSkip = 1, kCoopRobust = 2;
+// A slot is "A-dominated" when over the whole block tile 2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^kDomGap:
+// then Z_ij = A_j and 2cosh(R_j/T) = e^{R_j/T} to beyond fp64, so T ln Z_ij = R_j for every pair (neglected: < T 2^-56).
+constexpr int kDomGap = 58;
 
 template <int TH, int TD, int LH, int NW, int KB, int NB>
 struct CoopGeom {
@@ -71,9 +75,11 @@ struct CoopGeom {
   static constexpr int W = WD + LH * (TH + PADB);            // doubles per slot row
   static constexpr int SLOTS = KB * NB;        // slots per sub-batch
   static constexpr int BUF_DOUBLES = SLOTS * W + SLOTS;      // values + one int2 {eref, flags} per slot
+  static constexpr int HTOT = NT * NB + SLOTS;  // header array: dense slots compacted at the front (padded to whole
+                                               // sub-batches), A-dominated slots at the back
   static constexpr size_t smem_bytes =
-      sizeof(CoopHdr) * NT * NB + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
-      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8);
+      sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
+      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD) + sizeof(int) * 2 * (NW + 2);
   // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
   // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
   __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * (2 * NTD) + (jg / TD) * 2 + (jg & 1); }
@@ -95,14 +101,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   static_assert(WD % NT == 0 && NT % WH == 0, "P1 mapping");
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  CoopHdr* const hdr_s = reinterpret_cast<CoopHdr*>(smem_raw);                       // [NT*NB]
-  double* const buf_s = reinterpret_cast<double*>(hdr_s + NT * NB);                  // 2 x {[SLOTS][W] values, [SLOTS] int2}
+  CoopHdr* const hdr_s = reinterpret_cast<CoopHdr*>(smem_raw);                       // [HTOT]
+  double* const buf_s = reinterpret_cast<double*>(hdr_s + G::HTOT);                  // 2 x {[SLOTS][W] values, [SLOTS] int2}
   double* const tab256 = buf_s + 2 * G::BUF_DOUBLES;                                 // [256]
   double* const d2_s = tab256 + 256;                                                 // [WD]
   double* const h_s = d2_s + WD;                                                     // [WH]
   double* const rng_s = h_s + WH;                                                    // hmin hmax d2min d2max (+pad)
-  int* const ev_s = reinterpret_cast<int*>(rng_s + 8);                               // 2 x [SLOTS][W] (robust slots)
+  double* const accR_s = rng_s + 8;                                                  // [WD] sums of R_j over A-dominated slots
+  int* const ev_s = reinterpret_cast<int*>(accR_s + WD);                             // 2 x [SLOTS][W] (robust slots)
   int* const accE_s = ev_s + 2 * SLOTS * W;                                          // [TH*TD][NT]
+  int* const scan_s = accE_s + TH * TD * NT;                                         // [2][NW + 2] compaction scan
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int b = blockIdx.x;
@@ -118,6 +126,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   for (int i = tid; i < 256; i += NT) tab256[i] = P.tabs->exp2_j256[i];
   for (int i = tid; i < WD; i += NT) d2_s[i] = P.d2[min(td * WD + i, P.nd - 1)];
   for (int i = tid; i < WH; i += NT) h_s[i] = P.h[min(th * WH + i, P.nh - 1)];
+  for (int i = tid; i < WD; i += NT) accR_s[i] = 0.0;
   int* const myE = accE_s + tid;
 #pragma unroll
   for (int pq = 0; pq < TH * TD; ++pq) myE[pq * NT] = 0;
@@ -150,12 +159,17 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   const FactoredConsts& fc = P.fc;
   const unsigned long long kbeg = (unsigned long long)chunk * P.kc;
   const unsigned long long kend = min(P.nk, kbeg + P.kc);
-  const int nbatch = (int)((kend - kbeg + KB - 1) / KB);       // sub-batches of KB k-points (kc < 2^31 KB)
   const bool force_robust = (P.debug_flags & 1) != 0;
 
   // ---------------- P0: one k-point per thread -> NB slot headers (for NT consecutive k-points) ----------------
-  // returns (to every thread, through the barrier) whether any of the NT*NB slots needs the robust path
-  auto p0 = [&](int superbatch) -> bool {
+  // The NT*NB slots of a group are sorted into three kinds.  DENSE slots are compacted, in k order, to the front of
+  // hdr_s and padded with neutral skip slots to whole sub-batches of SLOTS; A-DOMINATED slots (early-out mode only)
+  // go to the back of hdr_s and are summed right here, sum_k R_j per Delta_j of the block tile, by the thread that
+  // owns Delta_j (no exponential, no pair work); skip slots (k past the chunk end, masked band) are dropped.
+  // Returns (to every thread, through the barriers) the number of dense sub-batches of the group and whether any
+  // of its dense slots needs the robust path.
+  const bool early_out = P.early_out != 0;
+  auto p0 = [&](int superbatch, int& nsub_out) -> bool {
     const unsigned long long kidx = kbeg + (unsigned long long)superbatch * NT + tid;
     const bool valid = kidx < kend;
     const unsigned long long kk = valid ? kidx : kbeg;
@@ -177,13 +191,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     if (FORM == 1) g2 *= ct.x * rr.x;
     g2 *= g2;
     bool any_robust = false;
+    CoopHdr hd[NB];
+    int kind[NB];                                            // 0 dropped, 1 dense, 2 A-dominated
+    int cnt = 0;                                             // dense count | dominated count << 16
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
-      CoopHdr hd;
       const double s = fma(0.5, Ek[e] + Eq[e], -P.mc.mu);    // (a + b)/2                  (S3)
       const double d0 = 0.5 * (Ek[e] - Eq[e]);               // (a - b)/2 + h
       const double s2 = fma(s, s, 1e-300);
-      hd.s2 = s2; hd.g2 = g2; hd.d0 = d0;
+      hd[e].s2 = s2; hd[e].g2 = g2; hd[e].d0 = d0;
       // exponent bounds over the block tile: R in [R(d2min), R(d2max)], |d0 - h| in [ymin, ymax]
       const double Rmax = sqrt_pos(fma(d2max, g2, s2));
       const double Rmin = sqrt_pos(fma(d2min, g2, s2));
@@ -196,24 +212,83 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const int hi = max(eAhi, eBhi) + 1, lo = max(eAlo, eBlo) - 1;
       const int spread = hi - lo;                            // every pair sum is in [2^lo, 2^(hi+2))
       const bool robust = force_robust || spread > kSpread;
-      hd.eref = hi - (spread >> 1);
-      int flags = robust ? (kCoopRobust | (3 << 8)) : (((spread >> 1) + 4) << 8);
-      if (!valid || !((P.mc.band_mask >> e) & 1)) { flags = kCoopSkip; hd.eref = 0; }
-      any_robust |= (flags & kCoopRobust) != 0;
-      hd.flags = flags;
-      hdr_s[tid * NB + e] = hd;
+      hd[e].eref = hi - (spread >> 1);
+      hd[e].flags = robust ? (kCoopRobust | (3 << 8)) : (((spread >> 1) + 4) << 8);
+      kind[e] = 1;
+      if (early_out && !force_robust && eAlo - eBhi >= kDomGap) kind[e] = 2;
+      if (!valid || !((P.mc.band_mask >> e) & 1)) kind[e] = 0;
+      any_robust |= kind[e] == 1 && robust;
+      cnt += kind[e] == 1 ? 1 : (kind[e] == 2 ? 0x10000 : 0);
     }
-    return __syncthreads_or(any_robust) != 0;
+    // block-wide exclusive scan of (dense, dominated) counts in slot order (tid, e)
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += v;
+    }
+    if (lane == 31) scan_s[warp] = incl;
+    __syncthreads();
+    int base = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const int v = scan_s[w];
+      if (w < warp) base += v;
+      total += v;
+    }
+    const int ndense = total & 0xffff, ndom = total >> 16;
+    const int nsub = (ndense + SLOTS - 1) / SLOTS;
+    int pd = (base + incl - cnt) & 0xffff;                   // first dense position of this thread
+    int pm = G::HTOT - ndom + ((base + incl - cnt) >> 16);   // first dominated position
+#pragma unroll
+    for (int e = 0; e < NB; ++e) {
+      if (kind[e] == 1) hdr_s[pd++] = hd[e];
+      else if (kind[e] == 2) hdr_s[pm++] = hd[e];
+    }
+    if (tid < nsub * SLOTS - ndense) {                       // neutral padding of the last sub-batch
+      CoopHdr z;
+      z.s2 = 1.0; z.g2 = 0.0; z.d0 = 0.0; z.eref = 0; z.flags = kCoopSkip;
+      hdr_s[ndense + tid] = z;
+    }
+    const bool rob = __syncthreads_or(any_robust) != 0;
+    // A-dominated slots: T ln Z_ij = R_j for the whole tile (kDomGap); this thread owns Delta_j, j = tid + r NT
+    if (ndom > 0) {
+      const CoopHdr* const dm = hdr_s + (G::HTOT - ndom);
+#pragma unroll 1
+      for (int r = 0; r < WD / NT; ++r) {
+        const double d2 = d2_s[tid + r * NT];
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;       // four independent sqrt chains, fixed order
+        int i = 0;
+#pragma unroll 1
+        for (; i + 4 <= ndom; i += 4) {
+          const double2 g0 = *reinterpret_cast<const double2*>(&dm[i].s2);
+          const double2 g1 = *reinterpret_cast<const double2*>(&dm[i + 1].s2);
+          const double2 g2v = *reinterpret_cast<const double2*>(&dm[i + 2].s2);
+          const double2 g3 = *reinterpret_cast<const double2*>(&dm[i + 3].s2);
+          a0 += sqrt_pos(fma(d2, g0.y, g0.x));               // R_j, Eq. 4 radicand           (S5)
+          a1 += sqrt_pos(fma(d2, g1.y, g1.x));
+          a2 += sqrt_pos(fma(d2, g2v.y, g2v.x));
+          a3 += sqrt_pos(fma(d2, g3.y, g3.x));
+        }
+        for (; i < ndom; ++i) {
+          const double2 g0 = *reinterpret_cast<const double2*>(&dm[i].s2);
+          a0 += sqrt_pos(fma(d2, g0.y, g0.x));
+        }
+        accR_s[tid + r * NT] += (a0 + a1) + (a2 + a3);
+      }
+    }
+    nsub_out = nsub;
+    return rob;
   };
 
-  // ---------------- P1: the SLOTS x (WD + WH) exponentials of sub-batch `bt` into buffer bt & 1 ----------------
+  // ---------------- P1: the SLOTS x (WD + WH) exponentials of sub-batch `j` of the group into buffer `par` ----------------
   // A thread keeps its Delta_j^2 (WD/NT of them) and its h_i and walks the slots, U independent chains at a time.
   // ROB: some slot of this group of NT k-points is robust -> per-slot flag test, robust slots store (m, e).
-  auto p1 = [&](int bt, auto rob_tag) {
+  auto p1 = [&](int j, int par, auto rob_tag) {
     constexpr bool ROB = decltype(rob_tag)::value;
-    const CoopHdr* const hdr_b = hdr_s + (bt % BPS) * SLOTS;
-    double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
-    int* const ev = ev_s + (bt & 1) * SLOTS * W;
+    const CoopHdr* const hdr_b = hdr_s + j * SLOTS;
+    double* const val = buf_s + par * G::BUF_DOUBLES;
+    int* const ev = ev_s + par * SLOTS * W;
     if (tid < SLOTS) reinterpret_cast<int2*>(val + SLOTS * W)[tid] = make_int2(hdr_b[tid].eref, hdr_b[tid].flags);
     // skip slots (k past the end of the chunk, masked band) get the neutral pair A' = 1, B' = 0: factor exactly 1
     auto put = [&](int pos, double m, int e, int eref, int flags, double neutral) {
@@ -288,8 +363,24 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     }
   };
 
-  bool sb_robust = p0(0);
-  if (sb_robust) p1(0, std::true_type{}); else p1(0, std::false_type{});
+  // Sub-batches are consumed group by group; a group (NT k-points) has `nsub` dense sub-batches after compaction,
+  // possibly none.  `next_group` runs P0 on the following groups until one has dense work (or the chunk ends).
+  const int ngroups = (int)((kend - kbeg + NT - 1) / NT);
+  int group_next = 0;                            // next group P0 has not seen yet
+  auto next_group = [&](int& nsub_out, bool& robust_out) -> bool {
+    while (group_next < ngroups) {
+      int ns = 0;
+      const bool rob = p0(group_next++, ns);
+      if (ns > 0) { nsub_out = ns; robust_out = rob; return true; }
+    }
+    return false;
+  };
+  int nsub = 0;                                  // dense sub-batches of the current group
+  bool sb_robust = false;
+  bool cur_exists = next_group(nsub, sb_robust);
+  if (cur_exists) {
+    if (sb_robust) p1(0, 0, std::true_type{}); else p1(0, 0, std::false_type{});
+  }
   __syncthreads();
 
   constexpr int HC = TH / 2;                     // the h half-tile handled between two shared-memory fetches
@@ -326,17 +417,21 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   int2 efn = make_int2(0, 0);
   bool have_s1 = false;
   bool cur_robust = sb_robust;                   // robust slots among the group of the sub-batch being consumed
+  int j = 0, par = 0;                            // current sub-batch: index in its group, buffer it sits in
 #pragma unroll 1
-  for (int bt = 0; bt < nbatch; ++bt) {
-    bool nxt_robust = cur_robust;
-    if (bt + 1 < nbatch && (bt + 1) % BPS == 0) nxt_robust = p0((bt + 1) / BPS);   // next sub-batch: new group of NT k
-    const bool fused = !cur_robust && !nxt_robust;
-    if (!fused && bt + 1 < nbatch) {
-      if (nxt_robust) p1(bt + 1, std::true_type{}); else p1(bt + 1, std::false_type{});
+  while (cur_exists) {
+    // the sub-batch after this one: the next of the same group, else the first of the next group with dense work
+    // (P0 may overwrite the headers now: P1 of every sub-batch of the current group is complete)
+    bool nxt_robust = cur_robust, nxt_exists = true;
+    int jn = j + 1, nsub_n = nsub;
+    if (jn == nsub) { jn = 0; nxt_exists = next_group(nsub_n, nxt_robust); }
+    const bool fused = !cur_robust && !(nxt_exists && nxt_robust);
+    if (!fused && nxt_exists) {
+      if (nxt_robust) p1(jn, par ^ 1, std::true_type{}); else p1(jn, par ^ 1, std::false_type{});
     }
-    // ---------------- P2: TH x TD pairs per thread and slot, from buffer bt & 1 ----------------
-    const double* const val = buf_s + (bt & 1) * G::BUF_DOUBLES;
-    const int* const ev = ev_s + (bt & 1) * SLOTS * W;
+    // ---------------- P2: TH x TD pairs per thread and slot, from buffer `par` ----------------
+    const double* const val = buf_s + par * G::BUF_DOUBLES;
+    const int* const ev = ev_s + par * SLOTS * W;
     const int2* const efs = reinterpret_cast<const int2*>(val + SLOTS * W);
     const double* const va0 = val + tdx * 2;                          // + sl W + p 2 NTD
     const double* const vb0 = val + WD + thx * (TH + G::PADB);        // + sl W + i
@@ -359,10 +454,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     load_b(b0, 0, 0);
 
     if (fused) {
-      // next sub-batch's headers and buffer ((bt + 1) may not exist: then this writes the idle buffer from stale,
+      // next sub-batch's headers and buffer (it may not exist: then this writes the idle buffer from stale,
       // finite headers, which nobody reads)
-      const CoopHdr* const hdr_n = hdr_s + ((bt + 1) % BPS) * SLOTS;
-      double* const valn = buf_s + ((bt + 1) & 1) * G::BUF_DOUBLES;
+      const CoopHdr* const hdr_n = hdr_s + jn * SLOTS;
+      double* const valn = buf_s + (par ^ 1) * G::BUF_DOUBLES;
       if (tid < SLOTS) reinterpret_cast<int2*>(valn + SLOTS * W)[tid] = make_int2(hdr_n[tid].eref, hdr_n[tid].flags);
       // The P1 chains are split in two stages that run one slot apart, so that each is short and independent of
       // the other: stage 1 (sqrt, range reduction) of slot sl + 1 and stage 2 (polynomial, scaling, store) of slot sl.
@@ -377,8 +472,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
           ta[r] = fma(xa[r], fc.c1, MAGIC);
         }
       }
-      const bool carry = (bt + 2) % BPS != 0;                         // sub-batch bt + 2 shares bt + 1's header group
-      const CoopHdr* const hdr_nn = hdr_s + ((bt + 2) % BPS) * SLOTS;
+      const bool carry = nxt_exists && jn + 1 < nsub_n;               // the sub-batch after next shares its header group
+      const CoopHdr* const hdr_nn = hdr_s + (jn + 1) * SLOTS;
       double mb = 0.0, xb = 0.0, tb = 0.0;
       int2 efb = make_int2(0, 0);
       const double* pa = va0;                                         // this thread's A' / B' of the current slot
@@ -521,8 +616,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
         for (int j = 0; j < TD; ++j) a[j] = an[j];
       }
     }
-    cur_robust = nxt_robust;
-    __syncthreads();     // buffer bt & 1 may be rewritten (by P1 of sub-batch bt + 2), buffer (bt + 1) & 1 is complete
+    cur_robust = nxt_robust; cur_exists = nxt_exists; j = jn; nsub = nsub_n; par ^= 1;
+    __syncthreads();     // buffer `par ^ 1` may be rewritten (by P1 of the sub-batch after next), buffer `par` is complete
   }
 
   // P_ij = T (ln2 * exponent sum + ln accP_ij); every thread owns its (h, Delta) pairs for the whole chunk
@@ -540,7 +635,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] - 1023 * nrenorm + ex);
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(mant)));
       if (ih < P.nh && id < P.nd)
-        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = P.T * lnz;
+        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = fma(P.T, lnz, accR_s[tdx * TD + j]);
     }
   }
 }

@@ -21,7 +21,7 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
 def run_gpu(fe, w, T, mode=None, tile=0, target_blocks=0, flags=0, shape=0):
-    """mode None = the library default (FE_EVAL_COOP, falling back to FACTORED on tiny grids); shape > 0 forces a
+    """mode None = the library default (FE_EVAL_COOP_EO, falling back to FACTORED on tiny grids); shape > 0 forces a
     block shape of the cooperative kernel (and with it the cooperative kernel itself)."""
     import torch
     with fe.FreeEnergy(w.params, w.N, T) as F:
@@ -169,7 +169,7 @@ def test_three_band_band_mask_const_mode_and_reuse(fe, oracle):
             torch.cuda.synchronize()
             ref = oracle.omega_grid(w.params, w.N, T, qs, w.h, w.delta)
             assert max_rel(om.cpu().numpy(), ref) < RTOL
-        assert F.last_launch_info()["mode"] == fe.EVAL_COOP
+        assert F.last_launch_info()["mode"] == fe.EVAL_COOP_EO
         with pytest.raises(fe.FeError):                      # per-thread kernels have no table path
             F.set_eval_mode(fe.EVAL_DIRECT)
             F.omega_grid(w.q, w.h, w.delta)
@@ -269,6 +269,44 @@ def test_pair_susceptibility_degenerate_and_errors(fe, oracle):
         om = F.omega_grid(w.q, w.h, w.delta)
         torch.cuda.synchronize()
         assert torch.isfinite(om).all()
+
+
+# ---- early-out variant of the cooperative kernel (FE_EVAL_COOP_EO, default): A-dominated slots summed as R_j ----
+@pytest.mark.parametrize("shape", [1, 2, 3, 4])
+def test_coop_early_out_parity_all_shapes(fe, oracle, shape):
+    cases = ((W.ragged(seed=23, N=70, nq=2, nh=11, nd=9), (0.004, 0.05, 1e-4)),
+             (W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=16, nd=32), (0.001, 0.01)),
+             (W.ragged(seed=29, N=50, nq=1, nh=9, nd=5, model=W.MODEL_ONE_BAND), (0.02,)),
+             (W.config(2), (0.001,)))
+    for w, temps in cases:
+        for T in temps:
+            om, ref = parity(fe, oracle, w, T, mode=fe.EVAL_COOP_EO, shape=shape)
+            dense = run_gpu(fe, w, T, mode=fe.EVAL_COOP, shape=shape)[0]
+            assert max_rel(om, dense) < 1e-13                       # same sums, two arithmetic routes
+
+
+def test_coop_early_out_extremes(fe, oracle):
+    # (a) every slot dominated: band far below the chemical potential (filled: Omega = sum 2 xi, not ~0), tiny fields
+    #     -> no dense sub-batch at all
+    p = W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(1.0,), mu=9.0, U=2.0)
+    w = W.Workload("all_dominated", p, 40, (0.002,), np.array([[0.1, 0.0], [0.0, 0.0]]), np.linspace(0, 0.05, 7),
+                   np.linspace(0, 0.3, 20))
+    parity(fe, oracle, w, 0.002, mode=fe.EVAL_COOP_EO, shape=1)
+    parity(fe, oracle, w, 0.002, mode=fe.EVAL_COOP_EO, shape=4)
+    # (b) nothing dominated: high temperature
+    w2 = W.interior_minimum(N=40, U=5.0, T=0.5, nq=2, nh=5, nd=12)
+    parity(fe, oracle, w2, 0.5, mode=fe.EVAL_COOP_EO, shape=1)
+    # (c) a masked band and a k-chunk tail shorter than a thread group (dropped slots), many k-chunks
+    w3 = W.Workload("masked", W.model_params(U=4.0, band_mask=2, cond_mult=1.0), 45, (0.003,),
+                    np.array([[0.3, -0.2]]), np.linspace(-0.05, 0.2, 9), np.linspace(0, 0.4, 21))
+    for tb in (1, 64, 4000):
+        parity(fe, oracle, w3, 0.003, mode=fe.EVAL_COOP_EO, shape=1, target_blocks=tb)
+    # (d) forced robust path switches the early-out off (debug flag 1) and still agrees
+    parity(fe, oracle, w3, 0.003, mode=fe.EVAL_COOP_EO, shape=3, flags=1)
+    # (e) bitwise determinism
+    a = run_gpu(fe, w3, 0.003, mode=fe.EVAL_COOP_EO, shape=1)[0]
+    b = run_gpu(fe, w3, 0.003, mode=fe.EVAL_COOP_EO, shape=1)[0]
+    assert np.array_equal(a, b)
 
 
 def test_factored_extreme_spreads(fe, oracle):
@@ -433,7 +471,7 @@ def load_golden(cfg):
     return json.load(open(path))
 
 
-@pytest.mark.parametrize("mode", [3, 0])
+@pytest.mark.parametrize("mode", [4, 3, 0])
 @pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_full_size_configs_sampled_parity(fe, cfg, mode):
     import torch
