@@ -43,6 +43,8 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 # cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
+    ("coop_eo", (64, 128)): (0.518, 0.652, "ncu, profiles/r1g_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.620 = 0.230 DADD + "
+                              "0.246 DMUL + 0.144 DFMA) and the T = 0.001 launch (0.416 = 0.138 + 0.153 + 0.125)"),
     ("coop", (64, 128)): (2.382, 2.668, "ncu, profiles/r1d_ksum_coop_64x128_raw.csv (1.036 DADD + 1.060 DMUL + 0.286 DFMA)"),
     ("coop", (64, 128), 3): (2.375, 2.656, "ncu, profiles/r1e_ksum_coop_3band_raw.csv (1.036 DADD + 1.059 DMUL + 0.281 DFMA)"),
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
@@ -53,7 +55,7 @@ KERNEL_COUNTS = {
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch from the ncu --set full capture in
 # profiles/ (a 1-q slice of the workload: 0.6 MB read, 95.5 MB written = the partial sums [ksplit][nh*nd]; the
 # launch timed here covers --q-per-step q-values and a different k-split, so this is context, not a bound: HBM is idle)
-KERNEL_TRAFFIC = {"coop": 96.1e6, ("coop", 3): 172.4e6}   # three-band: + 72 MB of band tables read
+KERNEL_TRAFFIC = {"coop_eo": 95.9e6, "coop": 96.1e6, ("coop", 3): 172.4e6}   # three-band: + 72 MB of band tables read
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
 PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
@@ -243,6 +245,7 @@ def main():
     ap.add_argument("--ref-deltas", type=int, default=64)
     ap.add_argument("--cpu-baseline-deltas", type=int, default=256)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-dense", action="store_true", help="skip the extra timing of the dense variant")
     ap.add_argument("--workload", default="omega", choices=["omega", "chi"],
                     help="omega = the free-energy scan (BASELINE.json metric); chi = pair-susceptibility q map (SURVEY 8f-4)")
     ap.add_argument("--chi-model", type=int, default=2)
@@ -339,6 +342,34 @@ def main():
     total_ms_max = float(t.item())
     value = evals_per_step * args.steps * world / (total_ms_max * 1e-3)
 
+    # ---- the dense variant of the same kernel (every pair multiplied out), timed beside the early-out default:
+    #      north_star's FP64-roofline target is read on it ----
+    dense = None
+    if args.mode == "coop_eo" and not args.no_dense:
+        F.set_eval_mode(fe.EVAL_COOP)
+        one_step(0); one_step(1)
+        barrier()
+        d_ms, dk_ms = [], []
+        for s in range(2):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            one_step(s)
+            e1.record(stream)
+            e1.synchronize()
+            d_ms.append(e0.elapsed_time(e1))
+            dk_ms.append(F.last_ksum()[0])
+        barrier()
+        dinfo = F.last_launch_info()
+        dc = KERNEL_COUNTS.get(("coop", (dinfo["th"], dinfo["td"]), w.nbands), KERNEL_COUNTS.get(("coop", (dinfo["th"], dinfo["td"]))))
+        dense = {"eval_mode": "coop", "steps": 2, "value": evals_per_step * 2 * world / (sum(d_ms) * 1e-3), "unit": UNIT,
+                 "ms_per_step": sum(d_ms) / 2, "ksum_ms": sum(dk_ms) / 2}
+        if dc:
+            ach = evals_per_step * w.nbands * dc[0] / (dense["ksum_ms"] * 1e-3) / 1e12
+            dense.update({"roofline_achieved": ach, "roofline_frac": ach / (PEAK_DFMA_PER_S / 1e12),
+                          "fp64_inst_per_band_eval": dc[0], "counts_source": dc[2]})
+        F.set_eval_mode(mode)
+
     # ---- e2e: host buffers through fe_scan_host (pinned), copies inside the timed region ----
     pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()    # noqa: E731
     out = dict(omega=pin((nq_step, w.nh, w.nd), torch.float64), idx=pin((nq_step, w.nh), torch.int32),
@@ -416,7 +447,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "api": "fe_scan_host (host buffers in/out, synchronous)"},
             "gpu_launches": launches, "wall_s_timed_region": t_wall, "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "result_check": idx_check}
+            "roofline": roofline, "dense_variant": dense, "cpu_baseline": cpu, "result_check": idx_check}
     del line["config"]["model"]
     print(json.dumps(line), flush=True)
     if world > 1:

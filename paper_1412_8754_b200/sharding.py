@@ -58,3 +58,34 @@ def scan_sharded(evaluate, q, h, delta, rank: int, world: int, group=None):
         ds = np.empty((0, nh))
         os_ = np.empty((0, nh))
     return gather_columns(idx, dict(idx=i, delta_star=ds, omega_star=os_), q.shape[0], rank, world, group)
+
+
+def combine_argmin_q(local_idx, iq_local, id_local, val_local, rank: int, world: int, group=None):
+    """Outer loop of Algorithm 1 (min over q) across ranks: every rank has run FreeEnergy.argmin_q on its own shard
+    (iq_local indexes the shard); the per-h winners are gathered (3 small arrays per rank) and reduced on the host
+    with the library's tie-break (lowest value, then lowest GLOBAL iq, then lowest Delta index).
+    Returns (iq, id, value) arrays of length nh, identical on every rank."""
+    import torch.distributed as dist
+    local_idx = np.asarray(local_idx, dtype=np.int64)
+    val = np.asarray(val_local, dtype=np.float64)
+    if len(local_idx):
+        giq = local_idx[np.asarray(iq_local, dtype=np.int64)]
+        payload = (giq, np.asarray(id_local, dtype=np.int64), val)
+    else:
+        payload = None
+    got = [payload]
+    if world > 1:
+        got = [None] * world
+        dist.all_gather_object(got, payload, group=group)
+    got = [g for g in got if g is not None]
+    nh = got[0][2].shape[0]
+    iq, idd, best = np.zeros(nh, np.int32), np.zeros(nh, np.int32), np.full(nh, np.inf)
+    first = np.ones(nh, dtype=bool)
+    for giq, gid, gval in got:
+        for ih in range(nh):
+            v = gval[ih]
+            better = v < best[ih] or (v == best[ih] and (giq[ih], gid[ih]) < (iq[ih], idd[ih]))
+            if (first[ih] and not np.isnan(v)) or better:
+                if not np.isnan(v):
+                    iq[ih], idd[ih], best[ih], first[ih] = giq[ih], gid[ih], v, False
+    return iq, idd, best

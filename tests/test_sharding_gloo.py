@@ -37,7 +37,13 @@ def _worker(rank, world, port, ret):
     out = sharding.scan_sharded(evaluate, w.q, w.h, w.delta, rank, world)
     # a rank with an empty shard must still take part (world > nq)
     out1 = sharding.scan_sharded(evaluate, w.q[:1], w.h, w.delta, rank, world)
+    # outer loop of Algorithm 1 across ranks: per-rank argmin over its q shard, then the tiny host-side combine
+    idx_q, qs = sharding.shard_q(w.q, rank, world)
+    om = O.omega_grid(w.params, w.N, w.T[0], qs, w.h, w.delta)
+    liq, lid, lval = O.argmin_q(om, ref_id=0)
+    giq, gid, gval = sharding.combine_argmin_q(idx_q, liq, lid, lval, rank, world)
     if rank == 0:
+        ret["gq"] = (giq, gid, gval)
         ret["idx"], ret["ds"], ret["os"] = out["idx"], out["delta_star"], out["omega_star"]
         ret["idx1"] = out1["idx"]
     dist.barrier()
@@ -59,6 +65,8 @@ def test_world2_sharded_scan_equals_single_process():
     idx, ds, os_ = O.argmin(om, w.delta)
     assert np.array_equal(ret["idx"], idx) and np.array_equal(ret["ds"], ds) and np.array_equal(ret["os"], os_)
     assert np.array_equal(ret["idx1"], idx[:1])
+    rq, rd, rv = O.argmin_q(om, ref_id=0)
+    assert np.array_equal(ret["gq"][0], rq) and np.array_equal(ret["gq"][1], rd) and np.array_equal(ret["gq"][2], rv)
 
 
 def test_world1_is_identity():
