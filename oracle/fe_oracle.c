@@ -388,3 +388,83 @@ int feo_pair_susceptibility(const feo_params* p, int32_t N, double T, const doub
     }
     return 0;
 }
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Single-precision variant ("the same CUDA C code in double precision (DP), single
+ * precision (SP), and single precision with fast intrinsic functions (SPFM)").
+ * The same Algorithm 1 / Eq. 4 / Eq. 5 as feo_omega_column with EVERY per-term operation in IEEE binary32
+ * (cosf, sinf, sqrtf, expf, log1pf; k, q, h, Delta, T, mu, hoppings rounded to float first).  Only the sum over k
+ * is kept in double (compensated), so that the result does not depend on summation order and can be compared
+ * (reading G20; the paper's kernel sums in float, order unspecified).  SPFM has no CPU counterpart (the
+ * "fast intrinsics" are GPU instructions): the SPFM kernel is compared with this function at a wider tolerance.
+ * One- and two-band models only.  Returns 0, -1 bad input, -2 allocation failure.
+ * --------------------------------------------------------------------------------------------------------- */
+static void feo_band_energies_sp(const feo_params* p, float kx, float ky, float* E) {
+    if (p->model == 1) {
+        E[0] = -2.0f * (float)p->t[0] * (cosf(kx) + cosf(ky));
+        return;
+    }
+    const float t1 = (float)p->t[0], t2 = (float)p->t[1], t3 = (float)p->t[2], t4 = (float)p->t[3];
+    const float T11 = -2.0f * (t1 * cosf(kx) + t2 * cosf(ky)) - 4.0f * t3 * cosf(kx) * cosf(ky);   /* A.1 */
+    const float T22 = -2.0f * (t2 * cosf(kx) + t1 * cosf(ky)) - 4.0f * t3 * cosf(kx) * cosf(ky);   /* A.2 */
+    const float T12 = -4.0f * t4 * sinf(kx) * sinf(ky);                                            /* A.3 */
+    const float avg = (T11 + T22) / 2.0f;
+    const float rad = sqrtf(((T11 - T22) / 2.0f) * ((T11 - T22) / 2.0f) + T12 * T12);
+    E[0] = avg + rad;                                                                              /* A.4 */
+    E[1] = avg - rad;
+}
+
+static float feo_thermal_sp(float x, float T) {          /* f(x) = -T ln(1 + exp(-x/T)), stable form, in float */
+    const float neg = x < 0.0f ? x : 0.0f;
+    return neg - T * log1pf(expf(-fabsf(x) / T));
+}
+
+int feo_omega_column_sp(const feo_params* p, int32_t N, double T, double qx, double qy, double h,
+                        const double* delta, int32_t nd, double* omega_out) {
+    if (!p || !delta || !omega_out || N < 1 || nd < 1 || !(T > 0.0) || !(p->U > 0.0)) return -1;
+    if (p->model != 1 && p->model != 2) return -1;
+    const int nb = feo_num_bands(p);
+    const size_t nk = (size_t)N * (size_t)N;
+    float* up  = (float*)malloc(sizeof(float) * nk * nb);
+    float* dn  = (float*)malloc(sizeof(float) * nk * nb);
+    float* cst = (float*)malloc(sizeof(float) * nk * nb);
+    float* eta = (float*)malloc(sizeof(float) * nk);
+    if (!up || !dn || !cst || !eta) { free(up); free(dn); free(cst); free(eta); return -2; }
+    const float Tf = (float)T, muf = (float)p->mu, hf = (float)h, qxf = (float)qx, qyf = (float)qy;
+    const float twopi = (float)(2.0 * M_PI);
+    for (int32_t j = 0; j < N; ++j)
+        for (int32_t i = 0; i < N; ++i) {
+            const float kx = twopi * (float)i / (float)N, ky = twopi * (float)j / (float)N;
+            float Ek[2], Ekq[2];
+            feo_band_energies_sp(p, kx, ky, Ek);
+            feo_band_energies_sp(p, -kx + qxf, -ky + qyf, Ekq);
+            const size_t k = (size_t)j * N + i;
+            eta[k] = p->form_factor == 0 ? (float)p->eta_scale : (float)p->eta_scale * cosf(kx) * cosf(ky);
+            for (int e = 0; e < nb; ++e) {
+                up[e * nk + k]  = Ek[e]  - muf - hf;
+                dn[e * nk + k]  = Ekq[e] - muf + hf;
+                cst[e * nk + k] = (p->const_mode == 0) ? dn[e * nk + k] : (Ek[e] - muf + hf);
+            }
+        }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t id = 0; id < nd; ++id) {
+        const float D = (float)delta[id];
+        feo_acc A = {0.0L, 0.0L};
+        for (int e = 0; e < nb; ++e) {
+            if (!((p->band_mask >> e) & 1)) continue;
+            for (size_t k = 0; k < nk; ++k) {
+                const float a = up[e * nk + k], b = dn[e * nk + k], gap = D * eta[k];
+                const float half_diff = (a - b) / 2.0f, half_sum = (a + b) / 2.0f;
+                const float root = sqrtf(half_sum * half_sum + gap * gap);                 /* Eq. 4 */
+                const float term = feo_thermal_sp(half_diff + root, Tf) + feo_thermal_sp(half_diff - root, Tf)
+                                 + cst[e * nk + k];                                        /* Eq. 5 */
+                acc_add(&A, (long double)term);
+            }
+        }
+        acc_add(&A, (long double)p->cond_mult * (long double)nk * (long double)delta[id] * (long double)delta[id]
+                        / (long double)p->U);
+        omega_out[id] = (double)(A.s + A.c);
+    }
+    free(up); free(dn); free(cst); free(eta);
+    return 0;
+}

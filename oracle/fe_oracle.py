@@ -58,6 +58,8 @@ def lib():
         L.feo_pair_term.restype = C.c_double
         L.feo_pair_susceptibility.argtypes = [pp, C.c_int32, C.c_double, dp, C.c_int32, C.c_double, dp]
         L.feo_pair_susceptibility.restype = C.c_int
+        L.feo_omega_column_sp.argtypes = L.feo_omega_column.argtypes
+        L.feo_omega_column_sp.restype = C.c_int
         L.feo_argmin_q.argtypes = [dp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, ip, ip, dp]
         L.feo_argmin_q.restype = C.c_int
         _lib = L
@@ -196,4 +198,22 @@ def pair_susceptibility(p: dict, N: int, T: float, q, h: float) -> np.ndarray:
     rc = lib().feo_pair_susceptibility(C.byref(sp), N, T, _dptr(q), q.shape[0], float(h), _dptr(out))
     if rc:
         raise ValueError(f"feo_pair_susceptibility failed: {rc}")
+    return out
+
+
+def omega_grid_sp(p: dict, N: int, T: float, q, h, delta) -> np.ndarray:
+    """Omega[iq, ih, id] with every per-term operation in binary32 (the paper's SP build; sum over k in double)."""
+    sp = _params(p)
+    q = np.ascontiguousarray(q, dtype=np.float64).reshape(-1, 2)
+    h = np.ascontiguousarray(h, dtype=np.float64).reshape(-1)
+    d = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+    out = np.empty((q.shape[0], h.shape[0], d.shape[0]), dtype=np.float64)
+    for iq in range(q.shape[0]):
+        for ih in range(h.shape[0]):
+            col = np.empty(d.shape[0])
+            rc = lib().feo_omega_column_sp(C.byref(sp), N, T, float(q[iq, 0]), float(q[iq, 1]), float(h[ih]), _dptr(d),
+                                           d.shape[0], _dptr(col))
+            if rc:
+                raise ValueError(f"feo_omega_column_sp failed: {rc}")
+            out[iq, ih] = col
     return out
