@@ -28,7 +28,9 @@ def test_sp_oracle_tracks_dp_oracle(oracle, w, T):
     srt = np.sort(dp, axis=-1)
     resolved = (srt[..., 1] - srt[..., 0]) > 16 * EPS32 * np.abs(srt[..., 0])
     assert np.array_equal(np.argmin(dp, -1)[resolved], np.argmin(sp, -1)[resolved])
-    assert resolved.sum() >= 1
+    # where the minimum is flatter than float resolution the SP index is still a DP near-minimum
+    pick = np.take_along_axis(dp, np.argmin(sp, -1)[..., None], -1)[..., 0]
+    assert np.all(pick - srt[..., 0] <= 8 * EPS32 * np.abs(srt[..., 0]))
 
 
 def test_sp_oracle_rejects_three_band_and_bad_input(oracle):
