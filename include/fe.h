@@ -147,6 +147,30 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
  * fe_get_timing reports (its second value is then the number of (k, q, e, f) pair terms).               */
 int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream);
 
+/* The paper's single-precision builds: Omega on the full grid with every per-term
+ * operation of Eq. 4 / Eq. 5 in binary32 -- fast_math = 0: "SP" (accurate expf / log1pf / sqrtf), 1: "SPFM" (fast
+ * intrinsics).  Only the sum over k is kept in double (fixed order).  Arguments as fe_omega_grid; omega_dev receives
+ * doubles.  One- and two-band models only (FE_EINVAL for the three-band model).  Expect ~1e-7 relative accuracy.  */
+int fe_omega_grid_sp(fe_handle* h,
+                     const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                     const double* delta, int32_t nd, int32_t fast_math,
+                     double* omega_dev, void* cuda_stream);
+
+/* Low-precision screening + selective double-precision verification ("run larger parameter scans at
+ * lower precision and then selectively verify with double precision calculations"):
+ *   1. fe_omega_grid_sp over the whole grid;  2. every Delta index that comes within margin_rel * |min| of the minimum
+ *   of ANY (q, h) column is a candidate;  3. fe_omega_grid (fp64, the handle's evaluation mode) on the candidate Delta
+ *   list only;  4. fe_argmin on that, indices mapped back to the full list.
+ * The minima equal those of a full fp64 scan whenever the single-precision error is below margin_rel / 2 (1e-5 is
+ * ample: measured error ~1e-7).  All list pointers HOST; idx_dev / delta_star_dev / omega_star_dev DEVICE, nq*nh each,
+ * any may be NULL; *n_verified_host (HOST, may be NULL) receives the number of Delta values evaluated in fp64.
+ * Synchronises the stream once between steps 2 and 3 (the candidate list is built on the host).            */
+int fe_scan_verified(fe_handle* h,
+                     const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                     const double* delta, int32_t nd, int32_t fast_math, double margin_rel,
+                     int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev,
+                     int32_t* n_verified_host, void* cuda_stream);
+
 /* Host-buffer end-to-end path: copies the lists to the device, runs fe_omega_grid and fe_argmin,
  * copies results back and SYNCHRONISES the stream.  All pointers are HOST memory (pinned or pageable).
  *   omega_host : nq*nh*nd doubles or NULL (skip the Omega copy-back);

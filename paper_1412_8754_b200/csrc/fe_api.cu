@@ -12,6 +12,7 @@
 #include "fe_kernels.cuh"
 #include "fe_bands3.cuh"
 #include "fe_chi.cuh"
+#include "fe_ksum_sp.cuh"
 #include "fe_launch.h"
 
 namespace {
@@ -72,6 +73,12 @@ struct fe_handle {
   size_t partial_cap = 0;
   double* d_spart = nullptr;
   size_t spart_cap = 0;
+  double* d_omega2 = nullptr;  // fe_scan_verified: fp64 Omega on the candidate Delta list
+  size_t omega2_cap = 0;
+  int32_t* d_flags = nullptr;  // fe_scan_verified: candidate flags per Delta index, then index scratch
+  size_t flags_cap = 0;
+  int32_t* h_flags = nullptr;  // pinned
+  size_t hflags_cap = 0;
   double* d_etab = nullptr;    // three-band model: [1 + nq][3][N*N] eigenvalue tables
   size_t etab_cap = 0;
   bool etab_base_valid = false;   // table 0 (unshifted grid) already computed for this handle
@@ -280,11 +287,16 @@ int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh
   return FE_OK;
 }
 
+// sp: 0 = the handle's fp64 evaluation mode; 1 = K1s SP; 2 = K1s SPFM (fe_ksum_sp.cuh)
 int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
-                    const double* delta, int32_t nd, double* omega_dev, cudaStream_t st) {
+                    const double* delta, int32_t nd, double* omega_dev, cudaStream_t st, int sp = 0) {
   const int N = h->N;
   // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
   int mode = h->mode;
+  if (sp) {
+    if (h->nb == 3) { snprintf(g_errbuf, sizeof g_errbuf, "the single-precision kernels cover the one- and two-band models"); return FE_EINVAL; }
+    mode = FE_EVAL_DIRECT;                                  // K1's geometry, tile (4, 4)
+  }
   int cshape = 0;
   const bool early_out = mode == FE_EVAL_COOP_EO;
   if (early_out) mode = FE_EVAL_COOP;                       // same kernel, CoopParams.early_out = 1
@@ -307,11 +319,11 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   }
   const bool coop = mode == FE_EVAL_COOP;
   // ---- stage lists: [q (2nq) | h (nh) | delta^2 (nd)] ----
-  const int tile = choose_tile_mode((mode == h->mode || (early_out && mode == FE_EVAL_COOP)) ? h->tile : 0, mode, nh, nd);
+  const int tile = sp ? 1 : choose_tile_mode((mode == h->mode || (early_out && mode == FE_EVAL_COOP)) ? h->tile : 0, mode, nh, nd);
   const int TH = kTiles[tile].th, TD = kTiles[tile].td;
   const int ntile_h = (nh + TH - 1) / TH;
   const int hstride = htile_stride(TH);
-  const size_t nlist = (size_t)2 * nq + nh + nd + (size_t)ntile_h * hstride;
+  const size_t nlist = (size_t)2 * nq + nh + nd + (size_t)ntile_h * hstride + (sp ? nd : 0);
   double *hs, *ds; StageSlot* slot;
   int rc = stage_lists(h, nlist, st, &hs, &ds, &slot);
   if (rc) return rc;
@@ -340,6 +352,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
       ht[3] = (double)fl;                          // eC (< 2^31: max|h|/T < 1e9 is enforced below)
     }
   }
+  if (sp) memcpy(hs + nlist - nd, delta, sizeof(double) * nd);       // K1s squares Delta in float itself
   FE_CUDA(cudaMemcpyAsync(ds, hs, nlist * sizeof(double), cudaMemcpyHostToDevice, st));
   FE_CUDA(cudaEventRecord(slot->ev, st));
   slot->pending = true;
@@ -462,7 +475,9 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     FE_CUDA(cudaGetLastError());
     h->launches++;
   }
-  if (h->nb == 3) {
+  if (sp) {
+    nschunk = 0;                                           // K1s sums the whole Eq. 5 term: no separate constant sum
+  } else if (h->nb == 3) {
     // KB: numerical band diagonalisation into the per-q tables (table 0 = unshifted grid, once per handle)
     Band3Consts bc;
     for (int i = 0; i < 12; ++i) bc.t[i] = h->p.tb3[i];
@@ -494,7 +509,22 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     CP.partial = h->d_partial; CP.etab = h->d_etab;
   }
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
-  if (coop) FE_CUDA(launch_coop(cshape, h->nb, h->p.form_factor, (int)grid_ll, st, CP));
+  if (sp) {
+    SpConsts sc;
+    for (int i = 0; i < 4; ++i) sc.t[i] = (float)h->p.t[i];
+    sc.mu = (float)h->p.mu; sc.eta_scale = (float)h->p.eta_scale; sc.T = (float)h->T;
+    P.d2 = ds + nlist - nd;                                // raw Delta list
+    const int g = (int)grid_ll, form = h->p.form_factor;
+#define FE_SP(NB_, F_, X_) fe_ksum_sp_kernel<NB_, F_, X_><<<g, kThreads, 0, st>>>(P, sc)
+    if (h->nb == 1) { if (form == 0) { if (sp == 2) FE_SP(1, 0, true); else FE_SP(1, 0, false); }
+                      else           { if (sp == 2) FE_SP(1, 1, true); else FE_SP(1, 1, false); } }
+    else            { if (form == 0) { if (sp == 2) FE_SP(2, 0, true); else FE_SP(2, 0, false); }
+                      else           { if (sp == 2) FE_SP(2, 1, true); else FE_SP(2, 1, false); } }
+#undef FE_SP
+    FE_CUDA(cudaGetLastError());
+    h->last_info[4] = 100 + sp;
+  }
+  else if (coop) FE_CUDA(launch_coop(cshape, h->nb, h->p.form_factor, (int)grid_ll, st, CP));
   else      FE_CUDA(launch_ksum(tile, h->nb, h->p.form_factor, mode, (int)grid_ll, st, P));
   h->launches++;
   if (h->timing) {
@@ -715,6 +745,68 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   return FE_OK;
 }
 
+int fe_omega_grid_sp(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                     const double* delta, int32_t nd, int32_t fast_math, double* omega_dev, void* cuda_stream) {
+  if (!h || !omega_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle or omega_dev is NULL"); return FE_EINVAL; }
+  if (fast_math != 0 && fast_math != 1) { snprintf(g_errbuf, sizeof g_errbuf, "fast_math must be 0 or 1"); return FE_EINVAL; }
+  int rc = check_lists(q_xy, nq, h_list, nh, delta, nd);
+  if (rc) return rc;
+  return omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, omega_dev, (cudaStream_t)cuda_stream, 1 + fast_math);
+}
+
+int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                     const double* delta, int32_t nd, int32_t fast_math, double margin_rel,
+                     int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev,
+                     int32_t* n_verified_host, void* cuda_stream) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (fast_math != 0 && fast_math != 1) { snprintf(g_errbuf, sizeof g_errbuf, "fast_math must be 0 or 1"); return FE_EINVAL; }
+  if (!(margin_rel >= 0.0) || !isfinite(margin_rel)) { snprintf(g_errbuf, sizeof g_errbuf, "margin_rel must be finite and >= 0"); return FE_EINVAL; }
+  int rc = check_lists(q_xy, nq, h_list, nh, delta, nd);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nout = (size_t)nq * nh * nd;
+  const int ncol = nq * nh;
+  if ((rc = ensure(h->d_omega, h->omega_cap, nout))) return rc;
+  if ((rc = ensure(h->d_flags, h->flags_cap, (size_t)(nd > ncol ? nd : ncol)))) return rc;
+  if ((size_t)nd > h->hflags_cap) {
+    if (h->h_flags) cudaFreeHost(h->h_flags);
+    h->h_flags = nullptr; h->hflags_cap = 0;
+    if (cudaMallocHost((void**)&h->h_flags, sizeof(int32_t) * (size_t)nd) != cudaSuccess) {
+      cudaGetLastError(); snprintf(g_errbuf, sizeof g_errbuf, "pinned allocation failed"); return FE_ENOMEM; }
+    h->hflags_cap = nd;
+  }
+  // 1. screening pass in single precision
+  if ((rc = omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, h->d_omega, st, 1 + fast_math))) return rc;
+  // 2. candidates
+  FE_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * (size_t)nd, st));
+  fe_mark_candidates_kernel<<<(ncol + 7) / 8, 256, 0, st>>>(ncol, nd, margin_rel, h->d_omega, h->d_flags);
+  FE_CUDA(cudaGetLastError());
+  h->launches++;
+  FE_CUDA(cudaMemcpyAsync(h->h_flags, h->d_flags, sizeof(int32_t) * (size_t)nd, cudaMemcpyDeviceToHost, st));
+  FE_CUDA(cudaStreamSynchronize(st));
+  int nu = 0;
+  for (int i = 0; i < nd; ++i) nu += h->h_flags[i] != 0;
+  if (nu == 0) { snprintf(g_errbuf, sizeof g_errbuf, "screening pass produced no finite minimum"); return FE_EINVAL; }
+  double* du = (double*)malloc(sizeof(double) * (size_t)nu);
+  if (!du) { snprintf(g_errbuf, sizeof g_errbuf, "host allocation failed"); return FE_ENOMEM; }
+  for (int i = 0, u = 0; i < nd; ++i) if (h->h_flags[i]) { du[u] = delta[i]; h->h_flags[u] = i; ++u; }   // u <= i: in place
+  if (n_verified_host) *n_verified_host = nu;
+  // 3. fp64 on the candidate list, 4. minima, mapped back
+  rc = ensure(h->d_omega2, h->omega2_cap, (size_t)ncol * nu);
+  if (!rc) rc = omega_grid_impl(h, q_xy, nq, h_list, nh, du, nu, h->d_omega2, st, 0);
+  if (!rc) rc = argmin_impl(h, h->d_omega2, du, ncol, nu, idx_dev, delta_star_dev, omega_star_dev, st);
+  free(du);
+  if (rc) return rc;
+  if (idx_dev) {
+    FE_CUDA(cudaMemcpyAsync(h->d_flags, h->h_flags, sizeof(int32_t) * (size_t)nu, cudaMemcpyHostToDevice, st));
+    fe_map_index_kernel<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, h->d_flags, idx_dev);
+    FE_CUDA(cudaGetLastError());
+    h->launches++;
+    FE_CUDA(cudaStreamSynchronize(st));        // h_flags (pinned map) may be reused by the next call
+  }
+  return FE_OK;
+}
+
 int fe_scan_host(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                  const double* delta, int32_t nd, double* omega_host, int32_t* idx_host,
                  double* delta_star_host, double* omega_star_host, void* cuda_stream) {
@@ -814,7 +906,8 @@ int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, d
 void fe_destroy(fe_handle* h) {
   if (!h) return;
   cudaFree(h->d_tabs); cudaFree(h->d_coltab); cudaFree(h->d_rowtab); cudaFree(h->d_partial);
-  cudaFree(h->d_spart); cudaFree(h->d_etab); cudaFree(h->d_omega); cudaFree(h->d_res);
+  cudaFree(h->d_spart); cudaFree(h->d_etab); cudaFree(h->d_omega); cudaFree(h->d_omega2); cudaFree(h->d_flags);
+  if (h->h_flags) cudaFreeHost(h->h_flags); cudaFree(h->d_res);
   for (auto& s : h->slots) {
     if (s.pending && s.ev) cudaEventSynchronize(s.ev);
     if (s.host) cudaFreeHost(s.host);

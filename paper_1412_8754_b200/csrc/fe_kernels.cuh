@@ -685,6 +685,32 @@ __global__ void __launch_bounds__(256) fe_argmin_q_kernel(int nq, int nh, int nd
 }
 
 // ---------------------------------------------------------------------------------------------------
+// K5 / K6 (fe_scan_verified: "run larger parameter scans at lower precision and then selectively verify with double
+// precision calculations").  K5: one warp per (q, h) column of the low-precision Omega: every Delta
+// index whose value is within margin_rel |min| of the column minimum is flagged (all writers store 1: benign).
+// K6: column minima found on the reduced (verified) Delta list are mapped back to indices of the full list.
+// ---------------------------------------------------------------------------------------------------
+__global__ void fe_mark_candidates_kernel(int ncol, int nd, double margin_rel, const double* __restrict__ omega,
+                                          int32_t* __restrict__ flags) {
+  const int col = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (col >= ncol) return;
+  const int lane = threadIdx.x & 31;
+  const double* om = omega + (size_t)col * nd;
+  double best = __longlong_as_double(0x7ff0000000000000LL);
+  for (int i = lane; i < nd; i += 32) best = fmin(best, om[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  const double thr = best + margin_rel * fabs(best);
+  for (int i = lane; i < nd; i += 32)
+    if (om[i] <= thr) flags[i] = 1;
+}
+
+__global__ void fe_map_index_kernel(int ncol, const int32_t* __restrict__ map, int32_t* __restrict__ idx) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < ncol) idx[c] = map[idx[c]];
+}
+
+// ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 16 independent DFMA chains per thread, register-resident.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) fe_dfma_probe_kernel(int iters, double seed, double* __restrict__ sink) {

@@ -16,7 +16,7 @@ from . import build as _build
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3, 4
 
-EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility", "fe_scan_host",
+EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility", "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host",
            "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info",
            "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
 
@@ -62,6 +62,9 @@ def lib():
     L.fe_argmin.argtypes = [vp, vp, dp, C.c_int32, C.c_int32, vp, vp, vp, vp]
     L.fe_argmin_q.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, vp]
     L.fe_pair_susceptibility.argtypes = [vp, dp, C.c_int32, C.c_double, vp, vp]
+    L.fe_omega_grid_sp.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, C.c_int32, vp, vp]
+    L.fe_scan_verified.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, C.c_int32, C.c_double, vp, vp, vp,
+                                   C.POINTER(C.c_int32), vp]
     L.fe_scan_host.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, vp, vp, vp, vp, vp]
     L.fe_enable_timing.argtypes = [vp, C.c_int32]
     L.fe_get_timing.argtypes = [vp, C.POINTER(C.c_float), dp]
@@ -256,6 +259,30 @@ class FreeEnergy:
         _check(lib().fe_pair_susceptibility(self._h, _dptr(q), q.shape[0], C.c_double(float(hz)),
                                             C.c_void_p(out.data_ptr()), _stream(stream)))
         return out
+
+    def omega_grid_sp(self, q, h, delta, fast_math=False, out=None, stream=None):
+        """Omega[iq, ih, id] from the single-precision kernels (the paper's SP / SPFM builds), as float64 tensor."""
+        import torch
+        q, h, d = _f64(q).reshape(-1, 2), _f64(h), _f64(delta)
+        if out is None:
+            out = torch.empty((q.shape[0], h.shape[0], d.shape[0]), dtype=torch.float64, device="cuda")
+        _check(lib().fe_omega_grid_sp(self._h, _dptr(q), q.shape[0], _dptr(h), h.shape[0], _dptr(d), d.shape[0],
+                                      int(bool(fast_math)), C.c_void_p(out.data_ptr()), _stream(stream)))
+        return out
+
+    def scan_verified(self, q, h, delta, fast_math=False, margin_rel=1e-5, stream=None):
+        """Single-precision screening + fp64 verification of the candidates: (idx, delta*, omega*, n_verified)."""
+        import torch
+        q, h, d = _f64(q).reshape(-1, 2), _f64(h), _f64(delta)
+        shp = (q.shape[0], h.shape[0])
+        idx = torch.empty(shp, dtype=torch.int32, device="cuda")
+        ds = torch.empty(shp, dtype=torch.float64, device="cuda")
+        os_ = torch.empty(shp, dtype=torch.float64, device="cuda")
+        nv = C.c_int32(0)
+        _check(lib().fe_scan_verified(self._h, _dptr(q), q.shape[0], _dptr(h), h.shape[0], _dptr(d), d.shape[0],
+                                      int(bool(fast_math)), float(margin_rel), C.c_void_p(idx.data_ptr()),
+                                      C.c_void_p(ds.data_ptr()), C.c_void_p(os_.data_ptr()), C.byref(nv), _stream(stream)))
+        return idx, ds, os_, nv.value
 
     def scan_host(self, q, h, delta, want_omega=True, out=None, stream=None):
         """Host-buffer end-to-end path (fe_scan_host): numpy in, numpy out, synchronous.

@@ -309,6 +309,61 @@ def test_coop_early_out_extremes(fe, oracle):
     assert np.array_equal(a, b)
 
 
+# ---- single-precision builds and screening + verification ----
+EPS32 = float(np.finfo(np.float32).eps)
+
+
+@pytest.mark.parametrize("fast", [False, True], ids=["SP", "SPFM"])
+def test_single_precision_kernels_vs_sp_oracle(fe, oracle, fast):
+    import torch
+    cases = ((W.config(1), 0.01), (W.config(2), 0.001), (W.interior_minimum(N=64, U=5.0, T=0.001, nq=3, nh=9, nd=37), 0.001),
+             (W.ragged(seed=7, N=45, nq=3, nh=5, nd=37), 0.004), (W.ragged(seed=29, N=50, nq=1, nh=9, nd=5, model=W.MODEL_ONE_BAND), 0.02))
+    for w, T in cases:
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            om = F.omega_grid_sp(w.q, w.h, w.delta, fast_math=fast)
+            om2 = F.omega_grid_sp(w.q, w.h, w.delta, fast_math=fast)
+            torch.cuda.synchronize()
+        assert torch.equal(om, om2)                                  # the k-sum is in double, fixed order
+        ref = oracle.omega_grid_sp(w.params, w.N, T, w.q, w.h, w.delta)
+        dp = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        err = max_rel(om.cpu().numpy(), ref)
+        # both sides evaluate the same float expressions; they differ in the trig values (correctly rounded float of the
+        # double table vs cosf: 1 ulp_32 of numbers up to the band width) and in expf/log1pf/sqrtf (1-2 ulp_32), SPFM in
+        # addition in the intrinsics' documented errors (__expf: 2 + |1.16 x| ulp_32 on terms already < e^{-|x|})
+        tol = (8 if not fast else 16) * EPS32
+        assert err < tol, f"{w.name} fast={fast}: {err:.3e} vs SP oracle"
+        assert max_rel(om.cpu().numpy(), dp) < 2 * tol             # and tracks the fp64 result to float accuracy
+
+
+@pytest.mark.parametrize("fast", [False, True], ids=["SP", "SPFM"])
+def test_scan_verified_equals_full_fp64_scan(fe, oracle, fast):
+    import torch
+    for w, T in ((W.interior_minimum(N=64, U=5.0, T=0.001, nq=4, nh=12, nd=160), 0.001),
+                 (W.ragged(seed=7, N=45, nq=3, nh=5, nd=37), 0.004), (W.config(2), 0.001)):
+        ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            idx, ds, os_, nver = F.scan_verified(w.q, w.h, w.delta, fast_math=fast)
+            om = F.omega_grid(w.q, w.h, w.delta)
+            fidx, fds, fos = F.argmin(om, w.delta)
+            torch.cuda.synchronize()
+        assert 1 <= nver <= w.nd
+        check_argmin(ref, w.delta, idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy())      # vs the fp64 oracle
+        # and against the library's own full fp64 scan: same minima wherever they are resolved
+        same = idx.cpu().numpy() == fidx.cpu().numpy()
+        assert np.all(np.abs(os_.cpu().numpy() - fos.cpu().numpy()) <= 1e-12 * np.abs(fos.cpu().numpy()))
+        assert same.mean() > 0.9
+    # a grid with well-separated interior minima really is thinned out by the screening
+    w = W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=4, nd=200)
+    with fe.FreeEnergy(w.params, w.N, 0.001) as F:
+        nver = F.scan_verified(w.q, w.h[:2], w.delta, fast_math=fast, margin_rel=1e-5)[3]
+        with pytest.raises(fe.FeError):
+            F.scan_verified(w.q, w.h, w.delta, margin_rel=-1.0)
+    assert nver < w.nd // 2, nver
+    with fe.FreeEnergy(W.three_band(N=16).params, 16, 0.01) as F3:
+        with pytest.raises(fe.FeError):
+            F3.omega_grid_sp([(0.0, 0.0)], [0.0], [0.0, 0.1])
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
