@@ -236,7 +236,7 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="coop_eo", choices=["coop_eo", "coop", "factored", "direct", "windowed"],
+    ap.add_argument("--mode", default="coop_eo", choices=["coop_eo", "coop", "factored", "direct", "windowed", "sp", "spfm", "verified_sp", "verified_spfm"],
                     help="coop_eo = library default (early-out); coop = dense variant (every pair multiplied out)")
     ap.add_argument("--shape", type=int, default=0, help="block shape of the cooperative kernel (0 = auto)")
     ap.add_argument("--config", type=int, default=4, help="4 = BASELINE.json headline config; 6 = same shape, three-band model")
@@ -281,7 +281,9 @@ def main():
     else:
         q_all = w.q
     temps = list(w.T)
-    mode = {"coop_eo": fe.EVAL_COOP_EO, "coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
+    sp_mode = args.mode in ("sp", "spfm", "verified_sp", "verified_spfm")       # the paper's SP / SPFM builds
+    mode = {"sp": fe.EVAL_COOP_EO, "spfm": fe.EVAL_COOP_EO, "verified_sp": fe.EVAL_COOP_EO, "verified_spfm": fe.EVAL_COOP_EO,
+            "coop_eo": fe.EVAL_COOP_EO, "coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
             "windowed": fe.EVAL_WINDOWED}[args.mode]
 
     F = fe.FreeEnergy(w.params, w.N, temps[0])
@@ -297,9 +299,18 @@ def main():
         s = (step * nq_step) % len(q_all)
         return np.ascontiguousarray(np.take(q_all, range(s, s + nq_step), axis=0, mode="wrap"))
 
+    verified_n = []
+
     def one_step(step):
         F.set_temperature(temps[step % len(temps)])
-        F.omega_grid(q_of(step), w.h, w.delta, out=omega, stream=stream)
+        if args.mode in ("sp", "spfm"):
+            F.omega_grid_sp(q_of(step), w.h, w.delta, fast_math=args.mode == "spfm", out=omega, stream=stream)
+        elif sp_mode:
+            r = F.scan_verified(q_of(step), w.h, w.delta, fast_math=args.mode == "verified_spfm", stream=stream)
+            verified_n.append(r[3])
+            return r[:3]
+        else:
+            F.omega_grid(q_of(step), w.h, w.delta, out=omega, stream=stream)
         return F.argmin(omega, w.delta, stream=stream)
 
     def barrier():
@@ -381,6 +392,8 @@ def main():
     e2e_steps = max(1, min(args.steps, 2))
     F.set_temperature(temps[0])
     hq[0][:] = q_of(0)
+    if sp_mode:
+        F.set_eval_mode(fe.EVAL_COOP_EO)       # e2e below is the fp64 host path; the SP numbers are the device-timed ones
     F.scan_host(hq[0], hh, hd, out=out, stream=stream)              # warm-up
     barrier()
     t0 = time.perf_counter()
@@ -420,6 +433,10 @@ def main():
                 "peak_measured_dfma_probe": dfma_rate / 1e12, "avg_launch_ms": k_ms,
                 "band_evals_per_launch": band_evals, "traffic": KERNEL_TRAFFIC.get((args.mode, w.nbands), KERNEL_TRAFFIC.get(args.mode)),
                 "kernel_share_of_step": k_ms * len(ksum_ms) / total_ms}
+    if sp_mode:
+        counts = (None, None, None)
+        roofline["note"] = ("single-precision builds (SURVEY 8f-2): FP32 / MUFU bound, see profiles/r1h_*; k_ms is the last k-sum launch "
+                            "(verified_*: the fp64 pass on the candidate list); candidates verified per step: " + str(verified_n[-4:]))
     if counts[0]:
         achieved = band_evals * counts[0] / (k_ms * 1e-3) / 1e12
         tflops = band_evals * counts[1] / (k_ms * 1e-3) / 1e12
