@@ -425,7 +425,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     bool nxt_robust = cur_robust, nxt_exists = true;
     int jn = j + 1, nsub_n = nsub;
     if (jn == nsub) { jn = 0; nxt_exists = next_group(nsub_n, nxt_robust); }
-    const bool fused = !cur_robust && !(nxt_exists && nxt_robust);
+    // exponent bookkeeping of the whole sub-batch at once (fused path): sum of the slots' reference exponents and of
+    // their drift steps; if the steps of one sub-batch alone could exceed the drift limit (very wide tiles at very
+    // low T) the sub-batch takes the plain path below, which checks the drift slot by slot
+    int sumE = 0, sumStep = 0;
+    {
+      const int2* const efc = reinterpret_cast<const int2*>(buf_s + par * G::BUF_DOUBLES + SLOTS * W);
+#pragma unroll
+      for (int sl = 0; sl < SLOTS; ++sl) { const int2 ef = efc[sl]; sumE += ef.x; sumStep += ef.y >> 8; }
+    }
+    const bool fused = !cur_robust && !(nxt_exists && nxt_robust) && sumStep <= kDriftLimit;
     if (!fused && nxt_exists) {
       if (nxt_robust) p1(jn, par ^ 1, std::true_type{}); else p1(jn, par ^ 1, std::false_type{});
     }
@@ -493,17 +502,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       };
 #pragma unroll
       for (int i = 0; i < QC; ++i) bq[0][i] = b0[i];
+      if (drift + sumStep > kDriftLimit) renorm();                    // skip slots: step 0, Eref 0, factors 1
+      drift += sumStep;
+      accEc += sumE;
 #pragma unroll 1
       for (int sl0 = 0; sl0 < SLOTS; sl0 += SPPE) {
         const int slB = slbB + (sl0 / SPPE) * SPP;                    // slot of this pass's B item
 #pragma unroll
         for (int us = 0; us < SPPE; ++us) {
           const int sl = sl0 + us;
-          const int2 ef = efs[sl];
-          const int step = ef.y >> 8;                                 // skip slots: step 0, Eref 0, factors 1
-          if (drift + step > kDriftLimit) renorm();
-          drift += step;
-          accEc += ef.x;
           // ---- one straight-line block: P2 of slot sl interleaved with the P1 chains for the next sub-batch ----
           double an[TD], ma[RA];
           int ea[RA];
