@@ -483,7 +483,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       }
       const bool carry = nxt_exists && jn + 1 < nsub_n;               // the sub-batch after next shares its header group
       const CoopHdr* const hdr_nn = hdr_s + (jn + 1) * SLOTS;
-      double mb = 0.0, xb = 0.0, tb = 0.0;
+      double mb = 0.0, xb = 0.0, tb = 0.0, vbB = 0.0;
+      int ebB = 0;
       int2 efb = make_int2(0, 0);
       const double* pa = va0;                                         // this thread's A' / B' of the current slot
       const double* pb = vb0;
@@ -552,6 +553,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
               }
               if (us == 0) mb = exp_mant(xb, tb, fc, tab256);
             }
+            if (c == NQ - 1 && us == 0) {                             // B_i: + e^{-|d|/T}, among the pair work of this chunk
+              ebB = exp_k(tb);
+              vbB = cosh_fix(mb, ebB);
+            }
 #pragma unroll
             for (int i = 0; i < QC; ++i)
 #pragma unroll
@@ -562,10 +567,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
             if (ea[r] < 28) ma[r] = cosh_fix(ma[r], ea[r]);           // + e^{-R/T} (rare)
             pvn[posAr[r]] = (efa.y & kCoopSkip) ? 1.0 : coop_scale(ma[r], ea[r] - efa.x);
           }
-          if (us == SPPE - 1) {                                       // B_i, stage 2
-            const int eb = exp_k(tb);
-            const double v = cosh_fix(mb, eb);
-            if (slB < SLOTS) valn[slB * W + posBr] = (efb.y & kCoopSkip) ? 0.0 : coop_scale(v, eb - efb.x);
+          if (us == SPPE - 1) {                                       // B_i, store
+            if (slB < SLOTS) valn[slB * W + posBr] = (efb.y & kCoopSkip) ? 0.0 : coop_scale(vbB, ebB - efb.x);
           }
 #pragma unroll
           for (int j = 0; j < TD; ++j) a[j] = an[j];
