@@ -43,9 +43,10 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 # cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
-    ("coop_eo", (64, 128)): (0.518, 0.652, "ncu, profiles/r1g_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.620 = 0.230 DADD + "
-                              "0.246 DMUL + 0.144 DFMA) and the T = 0.001 launch (0.416 = 0.138 + 0.153 + 0.125)"),
-    ("coop", (64, 128)): (2.382, 2.668, "ncu, profiles/r1d_ksum_coop_64x128_raw.csv (1.036 DADD + 1.060 DMUL + 0.286 DFMA)"),
+    ("coop_eo", (64, 128)): (0.521, 0.656, "ncu, profiles/r1k_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.624 = 0.231 DADD + "
+                              "0.248 DMUL + 0.145 DFMA) and the T = 0.001 launch (0.418 = 0.138 + 0.154 + 0.125)"),
+    ("coop_eo", (64, 128), 3): (0.299, 0.413, "ncu, profiles/r1k_ksum_coop_eo_3band_raw.csv (T = 0.001: 0.085 DADD + 0.101 DMUL + 0.113 DFMA)"),
+    ("coop", (64, 128)): (2.384, 2.669, "ncu, profiles/r1k_ksum_coop_dense_raw.csv (1.038 DADD + 1.061 DMUL + 0.285 DFMA)"),
     ("coop", (64, 128), 3): (2.375, 2.656, "ncu, profiles/r1e_ksum_coop_3band_raw.csv (1.036 DADD + 1.059 DMUL + 0.281 DFMA)"),
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
     ("factored", (16, 4)): (4.20, 5.62, "ncu, profiles/r1c_ksum_factored_16x4_raw.csv"),
@@ -55,7 +56,7 @@ KERNEL_COUNTS = {
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch from the ncu --set full capture in
 # profiles/ (a 1-q slice of the workload: 0.6 MB read, 95.5 MB written = the partial sums [ksplit][nh*nd]; the
 # launch timed here covers --q-per-step q-values and a different k-split, so this is context, not a bound: HBM is idle)
-KERNEL_TRAFFIC = {"coop_eo": 95.9e6, "coop": 96.1e6, ("coop", 3): 172.4e6}   # three-band: + 72 MB of band tables read
+KERNEL_TRAFFIC = {"coop_eo": 95.7e6, "coop": 96.5e6, ("coop", 3): 172.4e6, ("coop_eo", 3): 178.5e6}   # three-band: + 72 MB of band tables read
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
 PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
