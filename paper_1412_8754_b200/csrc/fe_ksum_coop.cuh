@@ -257,23 +257,27 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 #pragma unroll 1
       for (int r = 0; r < WD / NT; ++r) {
         const double d2 = d2_s[tid + r * NT];
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;       // four independent sqrt chains, fixed order
+        constexpr int UD = 8;                                // independent sqrt chains, fixed order
+        double acc[UD];
+        double2 g[UD];                                       // headers are fetched one round ahead of their use
+        auto ld = [&](int i) { return *reinterpret_cast<const double2*>(&dm[min(i, ndom - 1)].s2); };
+#pragma unroll
+        for (int u = 0; u < UD; ++u) { acc[u] = 0.0; g[u] = ld(u); }
         int i = 0;
 #pragma unroll 1
-        for (; i + 4 <= ndom; i += 4) {
-          const double2 g0 = *reinterpret_cast<const double2*>(&dm[i].s2);
-          const double2 g1 = *reinterpret_cast<const double2*>(&dm[i + 1].s2);
-          const double2 g2v = *reinterpret_cast<const double2*>(&dm[i + 2].s2);
-          const double2 g3 = *reinterpret_cast<const double2*>(&dm[i + 3].s2);
-          a0 += sqrt_pos(fma(d2, g0.y, g0.x));               // R_j, Eq. 4 radicand           (S5)
-          a1 += sqrt_pos(fma(d2, g1.y, g1.x));
-          a2 += sqrt_pos(fma(d2, g2v.y, g2v.x));
-          a3 += sqrt_pos(fma(d2, g3.y, g3.x));
+        for (; i + UD <= ndom; i += UD) {
+          double2 n[UD];
+#pragma unroll
+          for (int u = 0; u < UD; ++u) n[u] = ld(i + UD + u);
+#pragma unroll
+          for (int u = 0; u < UD; ++u) acc[u] += sqrt_pos(fma(d2, g[u].y, g[u].x));       // R_j, Eq. 4 radicand   (S5)
+#pragma unroll
+          for (int u = 0; u < UD; ++u) g[u] = n[u];
         }
-        for (; i < ndom; ++i) {
-          const double2 g0 = *reinterpret_cast<const double2*>(&dm[i].s2);
-          a0 += sqrt_pos(fma(d2, g0.y, g0.x));
-        }
+#pragma unroll
+        for (int u = 0; u < UD - 1; ++u)                     // tail: g[u] holds entry i + u (clamped loads)
+          if (i + u < ndom) acc[u] += sqrt_pos(fma(d2, g[u].y, g[u].x));
+        const double a0 = acc[0] + acc[4], a1 = acc[1] + acc[5], a2 = acc[2] + acc[6], a3 = acc[3] + acc[7];
         accR_s[tid + r * NT] += (a0 + a1) + (a2 + a3);
       }
     }
