@@ -484,7 +484,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     bc.e0 = h->p.tb3[12];
     const int y0 = h->etab_base_valid ? 1 : 0;
     dim3 g((unsigned)(((size_t)N * N + 255) / 256), (unsigned)(1 + nq - y0));
-    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, h->d_etab);
+    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, nullptr, h->d_etab);
     FE_CUDA(cudaGetLastError());
     h->etab_base_valid = true;
     h->launches++;
@@ -683,10 +683,23 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = h->N, nb = h->nb, nbb = nb * nb;
   double *hs, *ds; StageSlot* slot;
-  int rc = stage_lists(h, (size_t)2 * nq, st, &hs, &ds, &slot);
+  int rc = stage_lists(h, (size_t)3 * nq, st, &hs, &ds, &slot);
   if (rc) return rc;
   for (int i = 0; i < 2 * nq; ++i) hs[i] = -q_xy[i];          // tables of k - (-q) = k + q; E, eta even: = -k - q
-  FE_CUDA(cudaMemcpyAsync(ds, hs, (size_t)2 * nq * sizeof(double), cudaMemcpyHostToDevice, st));
+  int noff = 0;                                               // q-values off the k-grid: they need a band table each
+  for (int i = 0; i < nq; ++i) {                              // q on the k-grid: shift code sx + sy N, else -(table index)
+    const double mx = q_xy[2 * i] * N / (2.0 * 3.14159265358979323846), my = q_xy[2 * i + 1] * N / (2.0 * 3.14159265358979323846);
+    const double rx = nearbyint(mx), ry = nearbyint(my);
+    double code = -(double)(1 + noff);
+    if (fabs(mx - rx) <= 1e-9 && fabs(my - ry) <= 1e-9 && fabs(rx) < 1e15 && fabs(ry) < 1e15) {
+      const long long sx = (((long long)rx % N) + N) % N, sy = (((long long)ry % N) + N) % N;
+      code = (double)(sx + sy * (long long)N);
+    } else {
+      ++noff;
+    }
+    hs[2 * nq + i] = code;
+  }
+  FE_CUDA(cudaMemcpyAsync(ds, hs, (size_t)3 * nq * sizeof(double), cudaMemcpyHostToDevice, st));
   FE_CUDA(cudaEventRecord(slot->ev, st));
   slot->pending = true;
   const unsigned long long nk = (unsigned long long)N * N;
@@ -702,7 +715,7 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   if ((rc = ensure(h->d_rowtab, h->rowtab_cap, (size_t)nq * N))) return rc;
   if ((rc = ensure(h->d_partial, h->partial_cap, (size_t)nchunk * nq * nbb))) return rc;
   if (nb == 3) {
-    const size_t need = (size_t)(1 + nq) * 3 * N * N;
+    const size_t need = (size_t)(1 + noff) * 3 * N * N;
     if (need > h->etab_cap || !h->d_etab) h->etab_base_valid = false;
     if ((rc = ensure(h->d_etab, h->etab_cap, need))) return rc;
   }
@@ -715,7 +728,7 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
     bc.e0 = h->p.tb3[12];
     const int y0 = h->etab_base_valid ? 1 : 0;
     dim3 g((unsigned)((nk + 255) / 256), (unsigned)(1 + nq - y0));
-    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, h->d_etab);
+    fe_bands3_kernel<<<g, 256, 0, st>>>(bc, N, y0, h->d_coltab, h->d_rowtab, ds + 2 * nq, h->d_etab);
     FE_CUDA(cudaGetLastError());
     h->etab_base_valid = true;
     h->launches++;
@@ -724,7 +737,7 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   dim3 grid((unsigned)nchunk, (unsigned)nq);
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
   const int form = h->p.form_factor;
-#define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, h->d_partial)
+#define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, ds + 2 * nq, h->d_partial)
   if (nb == 1) { if (form == 0) FE_CHI(1, 0); else FE_CHI(1, 1); }
   else if (nb == 2) { if (form == 0) FE_CHI(2, 0); else FE_CHI(2, 1); }
   else { if (form == 0) FE_CHI(3, 0); else FE_CHI(3, 1); }

@@ -16,12 +16,32 @@ namespace fe {
 
 struct Band3Consts { double t[12]; double e0; };   // t[i-1] = t_i of PAPER.md:273
 
+// 1/x and 1/sqrt(x) for normal x without the slow-path branches of the IEEE division / sqrt: MUFU seed (~2^-22) and
+// two Newton steps (<= 1 ulp-level error; the rotation only has to be orthogonal to rounding accuracy).
+__device__ __forceinline__ double rcp_nr(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x * y, y, 1.0);                 // 1 - x y^2
+  y = fma(0.5 * y, e, y);
+  e = fma(-x * y, y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+
 __device__ __forceinline__ void jacobi_rotate(double& app, double& aqq, double& apq, double& arp, double& arq) {
   // zero a_pq; r is the third index.  t = tan(theta) of the smaller rotation angle.
-  if (apq == 0.0) return;
-  const double tau = (aqq - app) / (2.0 * apq);
-  const double t = copysign(1.0, tau) / (fabs(tau) + sqrt(fma(tau, tau, 1.0)));
-  const double c = rsqrt(fma(t, t, 1.0)), s = t * c;
+  if (fabs(apq) < 1e-280) { apq = 0.0; return; }    // (also keeps the reciprocal below finite)
+  double tau = (aqq - app) * rcp_nr(2.0 * apq);
+  tau = fmin(fmax(tau, -1e150), 1e150);             // tau^2 stays finite; t ~ 1/(2 tau) there
+  const double t = copysign(1.0, tau) * rcp_nr(fabs(tau) + sqrt_pos(fma(tau, tau, 1.0)));
+  const double c = rsqrt_nr(fma(t, t, 1.0)), s = t * c;
   app = fma(-t, apq, app);
   aqq = fma(t, apq, aqq);
   apq = 0.0;
@@ -62,21 +82,30 @@ __device__ __forceinline__ void band3_energies(const Band3Consts& bc, double cx,
 }
 
 // KB: grid = (ceil(N*N / 256), ny).  y0 = index of the first table this launch writes (0: the unshifted grid).
+// slot (nullable): slot[iq] >= 0 marks a q on the k-grid whose table is not needed (the caller reads table 0 shifted);
+// slot[iq] = -t < 0 sends the table of q_iq to table index t >= 1 (tables are then allocated for off-grid q only).
 __global__ void __launch_bounds__(256) fe_bands3_kernel(Band3Consts bc, int N, int y0,
                                                         const double4* __restrict__ coltab,
                                                         const double4* __restrict__ rowtab,
+                                                        const double* __restrict__ slot,
                                                         double* __restrict__ etab) {
   const size_t nk = (size_t)N * N;
   const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= nk) return;
   const int y = y0 + blockIdx.y;
+  int ytab = y;
+  if (y > 0 && slot) {
+    const double c = slot[y - 1];
+    if (c >= 0.0) return;
+    ytab = (int)(-c);
+  }
   const int row = (int)(k / (unsigned)N), col = (int)(k - (size_t)row * N);
   const int iq = y == 0 ? 0 : y - 1;
   const double4 ct = coltab[(size_t)iq * N + col], rt = rowtab[(size_t)iq * N + row];
   double E[3];
   if (y == 0) band3_energies(bc, ct.x, ct.y, rt.x, rt.y, E);
   else        band3_energies(bc, ct.z, ct.w, rt.z, rt.w, E);
-  double* out = etab + (size_t)y * 3 * nk + k;
+  double* out = etab + (size_t)ytab * 3 * nk + k;
   out[0] = E[0]; out[nk] = E[1]; out[2 * nk] = E[2];
 }
 

@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(kThreads) fe_chi_kernel(ModelConsts mc, double
                                                           const double4* __restrict__ coltab,
                                                           const double4* __restrict__ rowtab,
                                                           const double* __restrict__ etab,
+                                                          const double* __restrict__ shift,
                                                           double* __restrict__ partial) {
   const int iq = blockIdx.y, chunk = blockIdx.x;
   const unsigned long long nk = (unsigned long long)N * N;
@@ -60,10 +61,22 @@ __global__ void __launch_bounds__(kThreads) fe_chi_kernel(ModelConsts mc, double
     const double4 ct = coltab[(size_t)iq * N + col], rr = rowtab[(size_t)iq * N + row];
     double Ek[NB], Eq[NB];
     if constexpr (NB == 3) {
+      // q on the k-grid (the paper's FBZ map): E(k + q) is table 0 read at the shifted index, as in the paper's
+      // "generate matrices E for k in FBZ"; otherwise the per-q table built by fe_bands3_kernel
+      const double sc = shift[iq];
+      size_t base = (size_t)(-sc) * 3 * nk, kq = kk;           // off-grid: sc = -(table index)
+      if (sc >= 0.0) {
+        const long long code = (long long)sc;
+        const int sx = (int)(code % N), sy = (int)(code / N);
+        int c2 = col + sx, r2 = row + sy;
+        if (c2 >= N) c2 -= N;
+        if (r2 >= N) r2 -= N;
+        base = 0; kq = (size_t)r2 * N + c2;
+      }
 #pragma unroll
       for (int e = 0; e < 3; ++e) {
         Ek[e] = etab[(size_t)e * nk + kk];
-        Eq[e] = etab[((size_t)(1 + iq) * 3 + e) * nk + kk];
+        Eq[e] = etab[base + (size_t)e * nk + kq];
       }
     } else {
       band_energies<NB>(mc, ct.x, ct.y, rr.x, rr.y, Ek);     // E(k)

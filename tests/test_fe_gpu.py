@@ -259,6 +259,17 @@ def test_pair_susceptibility_degenerate_and_errors(fe, oracle):
             chi = F.pair_susceptibility([(0.0, 0.0), (np.pi, np.pi)], 0.0).cpu().numpy()
         ref = oracle.pair_susceptibility(p, N, T, [(0.0, 0.0), (np.pi, np.pi)], 0.0)
         assert max_rel(chi, ref) < RTOL
+    # three-band: q on the k-grid reads the unshifted band table at a shifted index, off-grid q gets a table of its
+    # own; a list mixing both (and negative / beyond-2pi grid vectors) exercises the slot bookkeeping
+    w3 = W.chi_map(model=3, N=24, nside=3, T=0.01, h=0.02)
+    g = 2 * np.pi / 24
+    qmix = np.array([[3 * g, 5 * g], [0.3, -0.2], [-2 * g, 30 * g], [0.0, 0.0], [1.1, 0.4], [23 * g, g]])
+    with fe.FreeEnergy(w3.params, 24, 0.01) as F:
+        chi = F.pair_susceptibility(qmix, 0.02).cpu().numpy()
+        chi_b = F.pair_susceptibility(qmix[::-1].copy(), 0.02).cpu().numpy()[::-1]
+    ref = oracle.pair_susceptibility(w3.params, 24, 0.01, qmix, 0.02)
+    assert np.max(np.abs(chi - ref) / np.abs(ref).max(axis=(1, 2), keepdims=True)) < 2e-12
+    assert np.max(np.abs(chi_b - chi) / np.abs(chi).max()) < 1e-14
     with fe.FreeEnergy(p, 8, 0.1) as F:
         with pytest.raises(fe.FeError):
             F.pair_susceptibility([(np.nan, 0.0)], 0.0)
