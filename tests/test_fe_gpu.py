@@ -375,6 +375,66 @@ def test_scan_verified_equals_full_fp64_scan(fe, oracle, fast):
             F3.omega_grid_sp([(0.0, 0.0)], [0.0], [0.0, 0.1])
 
 
+def test_randomised_grids_all_models(fe, oracle):
+    """Seeded random workloads (models, N odd / even, T over four decades, list lengths around the tile edges, q / h /
+    Delta of both signs, band masks, k-splits): default mode and the dense variant against the oracle."""
+    rng = np.random.default_rng(20141231)
+    for case in range(36):
+        model = int(rng.choice([1, 2, 3]))
+        N = int(rng.integers(5, 72))
+        T = float(10.0 ** rng.uniform(-4, 0))
+        nq, nh, nd = int(rng.integers(1, 4)), int(rng.choice([1, 3, 15, 16, 17, 33, 64, 65])), int(rng.choice([1, 7, 127, 128, 129, 140]))
+        if model == 3:
+            p = W.model_params(model=3, mu=W.THREE_BAND_MU + float(rng.uniform(-0.2, 0.2)), U=float(rng.uniform(0.8, 2.0)))
+            hs, ds, qs = 0.08, 0.2, 0.8
+        elif model == 2:
+            p = W.model_params(U=float(rng.uniform(2, 6)), mu=W.TWO_BAND_MU + float(rng.uniform(-1, 1)),
+                               t=W.perturbed_hoppings(int(rng.integers(1, 99))))
+            hs, ds, qs = 0.4, 0.5, 0.8
+        else:
+            p = W.model_params(model=1, form_factor=int(rng.integers(0, 2)), t=(float(rng.uniform(0.5, 1.5)),),
+                               mu=float(rng.uniform(-3, 3)), U=float(rng.uniform(1, 5)))
+            hs, ds, qs = 0.5, 0.6, 1.5
+        nb = W.NBANDS[model]
+        if rng.random() < 0.3:
+            p = dict(p, band_mask=int(rng.integers(1, 1 << nb)), const_mode=int(rng.integers(0, 2)))
+        w = W.Workload(f"rand{case}_m{model}_N{N}", p, N, (T,), rng.uniform(-qs, qs, size=(nq, 2)),
+                       np.sort(rng.uniform(-0.3 * hs, hs, size=nh)), np.sort(rng.uniform(-0.2 * ds, ds, size=nd)))
+        tb = int(rng.choice([0, 0, 1, 300]))
+        ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        # With a single, nearly empty band selected Omega(Delta) passes through zero along a column (the k-sum and the
+        # condensation term cancel), so the error is measured against the column's scale max_Delta |Omega|: that is
+        # the magnitude of the sums whose rounding the 1e-12 bound is about.
+        scale = np.abs(ref).max(axis=-1, keepdims=True)
+        for mode in (None, fe.EVAL_COOP):
+            om, idx, ds, os_ = run_gpu(fe, w, T, mode=mode, target_blocks=tb)
+            err = float(np.max(np.abs(om - ref) / scale))
+            assert err < RTOL, f"{w.name} mode={mode} T={T}: {err:.3e}"
+            assert np.array_equal(idx, np.argmin(om, axis=-1).astype(np.int32)) and np.array_equal(os_, om.min(axis=-1))
+
+
+def test_full_size_properties_in_bench_launch_configuration(fe):
+    """Whole config-3 and config-4 steps exactly as bench.py launches them (all q, all h, all Delta in one call):
+    properties that hold at any size -- Omega(q) = Omega(-q) (O4), the early-out and the dense variant agree, the
+    on-device minima are the minima of the device Omega, reruns are bit-identical."""
+    import torch
+    for cfg, T in ((3, 0.001), (4, 0.01)):
+        w = W.config(cfg)
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            a = F.omega_grid(w.q, w.h, w.delta)
+            idx, ds, os_ = F.argmin(a, w.delta)
+            a2 = F.omega_grid(w.q, w.h, w.delta)
+            b = F.omega_grid(-w.q, w.h, w.delta)
+            F.set_eval_mode(fe.EVAL_COOP)
+            c = F.omega_grid(w.q, w.h, w.delta)
+            torch.cuda.synchronize()
+            assert torch.equal(a, a2)
+            assert float(((a - b).abs() / a.abs()).max()) < 1e-12
+            assert float(((a - c).abs() / a.abs()).max()) < 1e-13
+            assert torch.equal(os_, a.min(dim=-1).values) and torch.equal(idx.long(), a.argmin(dim=-1))
+            assert bool(torch.isfinite(a).all())
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
