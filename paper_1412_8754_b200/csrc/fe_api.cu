@@ -737,7 +737,7 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   dim3 grid((unsigned)nchunk, (unsigned)nq);
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
   const int form = h->p.form_factor;
-#define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, ds + 2 * nq, h->d_partial)
+#define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, ds + 2 * nq, h->d_tabs, h->d_partial)
   if (nb == 1) { if (form == 0) FE_CHI(1, 0); else FE_CHI(1, 1); }
   else if (nb == 2) { if (form == 0) FE_CHI(2, 0); else FE_CHI(2, 1); }
   else { if (form == 0) FE_CHI(3, 0); else FE_CHI(3, 1); }

@@ -16,25 +16,6 @@ namespace fe {
 
 struct Band3Consts { double t[12]; double e0; };   // t[i-1] = t_i of PAPER.md:273
 
-// 1/x and 1/sqrt(x) for normal x without the slow-path branches of the IEEE division / sqrt: MUFU seed (~2^-22) and
-// two Newton steps (<= 1 ulp-level error; the rotation only has to be orthogonal to rounding accuracy).
-__device__ __forceinline__ double rcp_nr(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
-}
-__device__ __forceinline__ double rsqrt_nr(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-x * y, y, 1.0);                 // 1 - x y^2
-  y = fma(0.5 * y, e, y);
-  e = fma(-x * y, y, 1.0);
-  return fma(0.5 * y, e, y);
-}
-
 __device__ __forceinline__ void jacobi_rotate(double& app, double& aqq, double& apq, double& arp, double& arq) {
   // zero a_pq; r is the third index.  t = tan(theta) of the smaller rotation angle.
   if (fabs(apq) < 1e-280) { apq = 0.0; return; }    // (also keeps the reciprocal below finite)

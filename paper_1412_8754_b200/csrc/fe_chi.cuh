@@ -21,23 +21,24 @@ namespace fe {
 
 struct ChiSide { double x, ax, u, opu, th; };   // energy, |energy|, exp(-|x|/T), 1 + u, tanh(|x|/2T)
 
-__device__ __forceinline__ ChiSide chi_side(double x, double neg_beta) {
+__device__ __forceinline__ ChiSide chi_side(double x, double neg_beta, const MathTabs& tabs) {
   ChiSide s;
   s.x = x; s.ax = fabs(x);
   const double t = s.ax * neg_beta;            // -|x|/T <= 0
-  s.u = exp(t);                                // keeps its relative accuracy when tiny (w in the blocked pairs)
+  s.u = exp_nonpos(t, tabs);                   // branch-free (fe_math.cuh); keeps its relative accuracy when tiny
   const double em = t > -0.6931 ? expm1(t) : s.u - 1.0;   // u - 1 without cancellation for |x| << T (states on
   s.opu = 1.0 + s.u;                                      // the Fermi surface): tanh(|x|/2T) = (1-u)/(1+u)
-  s.th = -em / s.opu;
+  s.th = -em * rcp_nr(s.opu);
   return s;
 }
 
 __device__ __forceinline__ double chi_pair_factor(const ChiSide& a, const ChiSide& b, double inv2T) {
-  if (a.x * b.x > 0.0) return (a.th + b.th) / (2.0 * (a.ax + b.ax));
+  if (a.x * b.x > 0.0) return (a.th + b.th) * rcp_nr(2.0 * (a.ax + b.ax));
   const double z = fabs(a.x + b.x) * inv2T;
   const double w = fmax(a.u, b.u);
-  const double E = z > 20.0 ? 1.0 / z : (z == 0.0 ? 2.0 : -expm1(-2.0 * z) / z);
-  return w * E * inv2T / (a.opu * b.opu);
+  const double rz = rcp_nr(fmax(z, 1e-300));
+  const double E = z > 20.0 ? rz : (z == 0.0 ? 2.0 : -expm1(-2.0 * z) * rz);
+  return w * E * inv2T * rcp_nr(a.opu * b.opu);
 }
 
 // grid = (nchunk, nq), 256 threads.  partial[(chunk*nq + iq)*NB*NB + e*NB + f]
@@ -48,7 +49,11 @@ __global__ void __launch_bounds__(kThreads) fe_chi_kernel(ModelConsts mc, double
                                                           const double4* __restrict__ rowtab,
                                                           const double* __restrict__ etab,
                                                           const double* __restrict__ shift,
+                                                          const MathTabs* __restrict__ gtabs,
                                                           double* __restrict__ partial) {
+  __shared__ MathTabs tabs;                                  // only the 2^(j/64) table is used here
+  for (int i = threadIdx.x; i < kExpTabN; i += kThreads) tabs.exp2_j64[i] = gtabs->exp2_j64[i];
+  __syncthreads();
   const int iq = blockIdx.y, chunk = blockIdx.x;
   const unsigned long long nk = (unsigned long long)N * N;
   const unsigned long long k0 = (unsigned long long)chunk * kc, k1 = min(nk, k0 + kc);
@@ -88,8 +93,8 @@ __global__ void __launch_bounds__(kThreads) fe_chi_kernel(ModelConsts mc, double
     ChiSide A[NB], B[NB];
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
-      A[e] = chi_side(Ek[e] - mc.mu - hz, neg_beta);         // E_{eps k up}
-      B[e] = chi_side(Eq[e] - mc.mu + hz, neg_beta);         // E_{eps',-k-q,down}
+      A[e] = chi_side(Ek[e] - mc.mu - hz, neg_beta, tabs);         // E_{eps k up}
+      B[e] = chi_side(Eq[e] - mc.mu + hz, neg_beta, tabs);         // E_{eps',-k-q,down}
     }
 #pragma unroll
     for (int e = 0; e < NB; ++e)

@@ -67,6 +67,25 @@ __device__ __forceinline__ double sqrt_pos(double x) {
   return fma(g, r, g);
 }
 
+// 1/x and 1/sqrt(x) for normal x without the slow-path branches of the IEEE division / sqrt: MUFU seed (~2^-22) and
+// two Newton steps (<= 1 ulp-level error; the rotation only has to be orthogonal to rounding accuracy).
+__device__ __forceinline__ double rcp_nr(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x * y, y, 1.0);                 // 1 - x y^2
+  y = fma(0.5 * y, e, y);
+  e = fma(-x * y, y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Band energies at one k from its four trig values (S2).  E[0] = E_+, E[1] = E_- (A.4).
 // ---------------------------------------------------------------------------------------------------
