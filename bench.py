@@ -151,7 +151,7 @@ def run_reference(args, w):
 
 
 # FP64-pipe instructions per (k, q) point of the susceptibility kernel (all nb^2 band pairs), ncu (profiles/r1f_*)
-CHI_COUNTS = {(2,): (238.0, "ncu, profiles/r1f_chi_2band_raw.csv (153.0 DFMA + 43.4 DADD + 41.5 DMUL per (k, q) point, 4 band pairs)")}
+CHI_COUNTS = {(2,): (170.2, "ncu, profiles/r1m_chi_2band_raw.csv (89.2 DFMA + 36.5 DADD + 44.5 DMUL per (k, q) point, 4 band pairs)")}
 
 
 def run_chi(args):
