@@ -188,7 +188,9 @@ int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
 
 /* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode actually
- * used, rows per k-chunk}; for FE_EVAL_COOP: {WH, WD, ksplit, grid blocks, mode, k-points per chunk}.  Host-only. */
+ * used, rows per k-chunk}; for FE_EVAL_COOP / FE_EVAL_COOP_EO: {WH, WD, ksplit, grid blocks, mode, k-points per chunk};
+ * after fe_omega_grid_sp the mode entry is 101 (SP) or 102 (SPFM); after fe_pair_susceptibility
+ * {nb, nb, k-chunks, grid blocks, -1, k-points per chunk}.  Host-only. */
 int fe_get_last_launch_info(fe_handle* h, int32_t* info6);
 
 /* Number of kernel launches this handle has issued since creation (all kernels of this library). */
@@ -203,8 +205,9 @@ int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past th
  * resident blocks per SM}; FE_EINVAL past the end of the table. */
 int fe_set_coop_shape(fe_handle* h, int32_t shape);
 int fe_coop_shape_info(int32_t shape, int32_t* info6);
-/* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP: bit 0 = always take the robust per-pair path, bit 1 = never use the per-tile
- * h recurrence.  Results are the same sums; only the code path changes (lets tests cover each path).       */
+/* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP(_EO): bit 0 = always take the robust per-pair path (this also switches
+ * the early-out of FE_EVAL_COOP_EO off), bit 1 = never use the per-tile h recurrence (FACTORED).  Results are the same
+ * sums; only the code path changes (lets tests cover each path).                                            */
 int fe_set_debug_flags(fe_handle* h, int32_t flags);
 
 /* FP64 DFMA-chain microbenchmark on the current device (register-resident, no memory traffic):
