@@ -103,7 +103,7 @@ def test_ragged_two_band_all_tiles(fe, oracle, tile, mode):
 
 
 @pytest.mark.parametrize("flags", [0, 1])
-@pytest.mark.parametrize("shape", [1, 2, 3, 4])
+@pytest.mark.parametrize("shape", [1, 2, 3, 4, 5])
 def test_ragged_two_band_all_coop_shapes(fe, oracle, shape, flags):
     """The block-cooperative kernel on grids that divide no block tile (padding in h, Delta and the k-chunk tail),
     fast slots (flags 0) and every slot forced through the robust per-pair path (flags 1)."""
@@ -283,7 +283,7 @@ def test_pair_susceptibility_degenerate_and_errors(fe, oracle):
 
 
 # ---- early-out variant of the cooperative kernel (FE_EVAL_COOP_EO, default): A-dominated slots summed as R_j ----
-@pytest.mark.parametrize("shape", [1, 2, 3, 4])
+@pytest.mark.parametrize("shape", [1, 2, 3, 4, 5])
 def test_coop_early_out_parity_all_shapes(fe, oracle, shape):
     cases = ((W.ragged(seed=23, N=70, nq=2, nh=11, nd=9), (0.004, 0.05, 1e-4)),
              (W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=16, nd=32), (0.001, 0.01)),
