@@ -43,8 +43,8 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 # cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
-    ("coop_eo", (64, 128)): (0.521, 0.656, "ncu, profiles/r1k_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.624 = 0.231 DADD + "
-                              "0.248 DMUL + 0.145 DFMA) and the T = 0.001 launch (0.418 = 0.138 + 0.154 + 0.125)"),
+    ("coop_eo", (64, 128)): (0.5105, 0.644, "ncu, profiles/r1o_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.612 = 0.226 DADD + "
+                              "0.243 DMUL + 0.143 DFMA) and the T = 0.001 launch (0.409 = 0.135 + 0.150 + 0.124)"),
     ("coop_eo", (64, 128), 3): (0.299, 0.413, "ncu, profiles/r1k_ksum_coop_eo_3band_raw.csv (T = 0.001: 0.085 DADD + 0.101 DMUL + 0.113 DFMA)"),
     ("coop", (64, 128)): (2.384, 2.669, "ncu, profiles/r1k_ksum_coop_dense_raw.csv (1.038 DADD + 1.061 DMUL + 0.285 DFMA)"),
     ("coop", (64, 128), 3): (2.375, 2.656, "ncu, profiles/r1e_ksum_coop_3band_raw.csv (1.036 DADD + 1.059 DMUL + 0.281 DFMA)"),
