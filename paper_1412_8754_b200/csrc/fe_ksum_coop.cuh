@@ -79,7 +79,7 @@ struct CoopGeom {
                                                // sub-batches), A-dominated slots at the back
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
-      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD) + sizeof(int) * 2 * (NW + 2);
+      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT) + sizeof(int) * 2 * (NW + 2);
   // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
   // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
   __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * (2 * NTD) + (jg / TD) * 2 + (jg & 1); }
@@ -108,7 +108,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   double* const h_s = d2_s + WD;                                                     // [WH]
   double* const rng_s = h_s + WH;                                                    // hmin hmax d2min d2max (+pad)
   double* const accR_s = rng_s + 8;                                                  // [WD] sums of R_j over A-dominated slots
-  int* const ev_s = reinterpret_cast<int*>(accR_s + WD);                             // 2 x [SLOTS][W] (robust slots)
+  double* const accB_s = accR_s + WD;                                                // [NT / WH][WH] sums of |d_i| over B-dominated slots
+  int* const ev_s = reinterpret_cast<int*>(accB_s + NT);                             // 2 x [SLOTS][W] (robust slots)
   int* const accE_s = ev_s + 2 * SLOTS * W;                                          // [TH*TD][NT]
   int* const scan_s = accE_s + TH * TD * NT;                                         // [2][NW + 2] compaction scan
 
@@ -127,6 +128,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   for (int i = tid; i < WD; i += NT) d2_s[i] = P.d2[min(td * WD + i, P.nd - 1)];
   for (int i = tid; i < WH; i += NT) h_s[i] = P.h[min(th * WH + i, P.nh - 1)];
   for (int i = tid; i < WD; i += NT) accR_s[i] = 0.0;
+  accB_s[tid] = 0.0;
   int* const myE = accE_s + tid;
 #pragma unroll
   for (int pq = 0; pq < TH * TD; ++pq) myE[pq * NT] = 0;
@@ -165,7 +167,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   // The NT*NB slots of a group are sorted into three kinds.  DENSE slots are compacted, in k order, to the front of
   // hdr_s and padded with neutral skip slots to whole sub-batches of SLOTS; A-DOMINATED slots (early-out mode only)
   // go to the back of hdr_s and are summed right here, sum_k R_j per Delta_j of the block tile, by the thread that
-  // owns Delta_j (no exponential, no pair work); skip slots (k past the chunk end, masked band) are dropped.
+  // owns Delta_j (no exponential, no pair work), B-DOMINATED slots likewise as sum_k |d0 - h_i| per h_i; skip slots (k past the chunk end, masked band) are dropped.
   // Returns (to every thread, through the barriers) the number of dense sub-batches of the group and whether any
   // of its dense slots needs the robust path.
   const bool early_out = P.early_out != 0;
@@ -192,8 +194,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     g2 *= g2;
     bool any_robust = false;
     CoopHdr hd[NB];
-    int kind[NB];                                            // 0 dropped, 1 dense, 2 A-dominated
-    int cnt = 0;                                             // dense count | dominated count << 16
+    int kind[NB];                                            // 0 dropped, 1 dense, 2 A-dominated, 3 B-dominated
+    int cnt = 0;                                             // dense | A-dominated << 10 | B-dominated << 20 (each <= NT NB < 1024)
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
       const double s = fma(0.5, Ek[e] + Eq[e], -P.mc.mu);    // (a + b)/2                  (S3)
@@ -216,9 +218,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       hd[e].flags = robust ? (kCoopRobust | (3 << 8)) : (((spread >> 1) + 4) << 8);
       kind[e] = 1;
       if (early_out && !force_robust && eAlo - eBhi >= kDomGap) kind[e] = 2;
+      if (early_out && !force_robust && eBlo - eAhi >= kDomGap) kind[e] = 3;
       if (!valid || !((P.mc.band_mask >> e) & 1)) kind[e] = 0;
       any_robust |= kind[e] == 1 && robust;
-      cnt += kind[e] == 1 ? 1 : (kind[e] == 2 ? 0x10000 : 0);
+      cnt += kind[e] == 1 ? 1 : (kind[e] == 2 ? (1 << 10) : (kind[e] == 3 ? (1 << 20) : 0));
     }
     // block-wide exclusive scan of (dense, dominated) counts in slot order (tid, e)
     int incl = cnt;
@@ -236,14 +239,17 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       if (w < warp) base += v;
       total += v;
     }
-    const int ndense = total & 0xffff, ndom = total >> 16;
+    const int ndense = total & 0x3ff, ndom = (total >> 10) & 0x3ff, ndomB = total >> 20;
     const int nsub = (ndense + SLOTS - 1) / SLOTS;
-    int pd = (base + incl - cnt) & 0xffff;                   // first dense position of this thread
-    int pm = G::HTOT - ndom + ((base + incl - cnt) >> 16);   // first dominated position
+    const int off = base + incl - cnt;                       // exclusive prefix of the three counts
+    int pd = off & 0x3ff;                                    // first dense position of this thread
+    int pm = G::HTOT - ndom + ((off >> 10) & 0x3ff);         // first A-dominated position (back of the array)
+    int pb = G::HTOT - ndom - ndomB + (off >> 20);           // first B-dominated position (just before them)
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
       if (kind[e] == 1) hdr_s[pd++] = hd[e];
       else if (kind[e] == 2) hdr_s[pm++] = hd[e];
+      else if (kind[e] == 3) hdr_s[pb++] = hd[e];
     }
     if (tid < nsub * SLOTS - ndense) {                       // neutral padding of the last sub-batch
       CoopHdr z;
@@ -280,6 +286,21 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
         const double a0 = acc[0] + acc[4], a1 = acc[1] + acc[5], a2 = acc[2] + acc[6], a3 = acc[3] + acc[7];
         accR_s[tid + r * NT] += (a0 + a1) + (a2 + a3);
       }
+    }
+    // B-dominated slots (2cosh(|d_i|/T) exceeds 2cosh(R_j/T) by 2^kDomGap over the whole tile): T ln Z_ij = |d0 - h_i|
+    // for every Delta_j.  Thread (half, ib) = (tid / WH, tid % WH) sums every (NT / WH)-th entry for its h_i.
+    if (ndomB > 0) {
+      const CoopHdr* const db = hdr_s + (G::HTOT - ndom - ndomB);
+      const double hv = h_s[tid % WH];
+      double a0 = 0.0, a1 = 0.0;
+      int i = tid / WH;
+#pragma unroll 1
+      for (; i + NT / WH < ndomB; i += 2 * (NT / WH)) {
+        a0 += fabs(db[i].d0 - hv);
+        a1 += fabs(db[i + NT / WH].d0 - hv);
+      }
+      if (i < ndomB) a0 += fabs(db[i].d0 - hv);
+      accB_s[tid] += a0 + a1;
     }
     nsub_out = nsub;
     return rob;
@@ -640,6 +661,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 #pragma unroll
   for (int i = 0; i < TH; ++i) {
     const int ih = th * WH + thx * TH + i;
+    double sumB = 0.0;                                         // B-dominated slots, fixed order over the partial sums
+#pragma unroll
+    for (int hf = 0; hf < NT / WH; ++hf) sumB += accB_s[hf * WH + thx * TH + i];
 #pragma unroll
     for (int j = 0; j < TD; ++j) {
       const int id = td * WD + tdx * TD + j;
@@ -649,7 +673,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] - 1023 * nrenorm + ex);
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(mant)));
       if (ih < P.nh && id < P.nd)
-        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = fma(P.T, lnz, accR_s[tdx * TD + j]);
+        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = fma(P.T, lnz, accR_s[tdx * TD + j] + sumB);
     }
   }
 }

@@ -304,6 +304,16 @@ def test_coop_early_out_extremes(fe, oracle):
                    np.linspace(0, 0.3, 20))
     parity(fe, oracle, w, 0.002, mode=fe.EVAL_COOP_EO, shape=1)
     parity(fe, oracle, w, 0.002, mode=fe.EVAL_COOP_EO, shape=4)
+    # (a') large fields: slots near the Fermi surface are B-dominated (2cosh(|d|/T) >> 2cosh(R/T)), the band edges
+    #      A-dominated, a few in between dense; h lists that fill and that do not fill the h tile
+    for nh, nd, N in ((7, 20, 40), (64, 9, 33), (70, 130, 24)):
+        wb = W.Workload("b_dominated", W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(1.0,), mu=0.3, U=2.0),
+                        N, (0.002,), np.array([[0.1, 0.0], [0.7, -0.4]]), np.linspace(1.5, 2.2, nh), np.linspace(0, 0.05, nd))
+        for shape in (1, 2, 4, 5):
+            parity(fe, oracle, wb, 0.002, mode=fe.EVAL_COOP_EO, shape=shape)
+    wb2 = W.Workload("b_dominated2", W.model_params(U=4.0), 36, (0.001,), np.array([[0.2, 0.1]]),
+                     np.linspace(-0.9, 0.9, 33), np.linspace(0, 0.1, 40))
+    parity(fe, oracle, wb2, 0.001, mode=fe.EVAL_COOP_EO)
     # (b) nothing dominated: high temperature
     w2 = W.interior_minimum(N=40, U=5.0, T=0.5, nq=2, nh=5, nd=12)
     parity(fe, oracle, w2, 0.5, mode=fe.EVAL_COOP_EO, shape=1)
