@@ -43,20 +43,20 @@ UNIT = "k-point x (q,h,Delta) evaluations/s"
 # cfg4 launch (profiles/); direct: cuobjdump -sass count of the band-loop body (every term takes the same path).
 KERNEL_COUNTS = {
     # (eval mode, (TH, TD)): (fp64 pipe instructions, flops [DFMA = 2, DADD/DMUL = 1]) per band-eval, source
-    ("coop_eo", (64, 128)): (0.5105, 0.644, "ncu, profiles/r1o_ksum_coop_eo_raw.csv: mean of the T = 0.01 launch (0.612 = 0.226 DADD + "
-                              "0.243 DMUL + 0.143 DFMA) and the T = 0.001 launch (0.409 = 0.135 + 0.150 + 0.124)"),
-    ("coop_eo", (64, 128), 3): (0.299, 0.413, "ncu, profiles/r1k_ksum_coop_eo_3band_raw.csv (T = 0.001: 0.085 DADD + 0.101 DMUL + 0.113 DFMA)"),
-    ("coop", (64, 128)): (2.384, 2.669, "ncu, profiles/r1k_ksum_coop_dense_raw.csv (1.038 DADD + 1.061 DMUL + 0.285 DFMA)"),
+    ("coop_eo", (64, 128)): (0.5391, 0.6683, "ncu on the benchmark's own launches (whole 32-q step), profiles/r1p_fullstep_eo.csv: mean of the "
+                              "T = 0.01 launch (0.662 = 0.252 DADD + 0.269 DMUL + 0.141 DFMA) and the T = 0.001 launch (0.416 = 0.142 + 0.158 + 0.117)"),
+    ("coop_eo", (64, 128), 3): (0.3307, 0.4419, "ncu, whole step, profiles/r1p_fullstep_b3_eo.csv (T = 0.001: 0.102 DADD + 0.118 DMUL + 0.111 DFMA)"),
+    ("coop", (64, 128)): (2.368, 2.647, "ncu, whole step, profiles/r1p_fullstep_dense.csv (1.032 DADD + 1.057 DMUL + 0.279 DFMA)"),
     ("coop", (64, 128), 3): (2.375, 2.656, "ncu, profiles/r1e_ksum_coop_3band_raw.csv (1.036 DADD + 1.059 DMUL + 0.281 DFMA)"),
     ("factored", (8, 4)): (8.49, 13.31, "ncu, profiles/r1b_ksum_factored_8x4_raw.csv"),
     ("factored", (16, 4)): (4.20, 5.62, "ncu, profiles/r1c_ksum_factored_16x4_raw.csv"),
     ("direct", (4, 4)): (40.6, 61.3, "SASS count"),
     ("direct", (8, 4)): (39.4, 59.4, "SASS count"),
 }
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch from the ncu --set full capture in
-# profiles/ (a 1-q slice of the workload: 0.6 MB read, 95.5 MB written = the partial sums [ksplit][nh*nd]; the
-# launch timed here covers --q-per-step q-values and a different k-split, so this is context, not a bound: HBM is idle)
-KERNEL_TRAFFIC = {"coop_eo": 95.7e6, "coop": 96.5e6, ("coop", 3): 172.4e6, ("coop_eo", 3): 178.5e6}   # three-band: + 72 MB of band tables read
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE k-sum launch of the default whole-step benchmark
+# (profiles/r1p_fullstep_*.csv: ~10 MB read, ~255 MB written = the partial sums [ksplit][nq*nh*nd]; three-band: + 1.1 GB
+# of band tables read).  Against 6.5 TB/s this is < 1 % of the launch time: HBM is idle, the bound is the FP64 pipe.
+KERNEL_TRAFFIC = {"coop_eo": 265.0e6, "coop": 280.0e6, ("coop", 3): 1.40e9, ("coop_eo", 3): 1.404e9}   # whole-step launches (r1p_fullstep_*)
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_GHZ = 148, 64, 1.965
 PEAK_DFMA_PER_S = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_GHZ * 1e9        # 1.861e13 thread-level FP64 instr/s
 PEAK_TFLOPS = 2 * PEAK_DFMA_PER_S / 1e12                                  # 37.2 TFLOP/s nominal
