@@ -51,26 +51,18 @@ extern "C" {
 #define FE_FORM_S   0       /* eta(k) = eta_scale                       (homogeneous s-wave)                      */
 #define FE_FORM_SPM 1       /* eta(k) = eta_scale * cos kx * cos ky     (s+-)                        */
 
-/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); all five compute the same sums ----
- * COOP_EO : default.  COOP with a block-uniform early-out: a (k, band) slot whose 2cosh(R_j/T) exceeds 2cosh(|d_i|/T)
- *           by more than 2^58 over the whole block tile contributes T ln Z_ij = R_j (exact to fp64), so it is summed
- *           per Delta_j without exponentials or pair products; the other slots are compacted and run through COOP's
- *           dense pipeline.  Same results to ~1e-15 relative; several times fewer FP64 instructions at low T.
- * COOP    : the dense variant (every pair of every slot is multiplied out).  The factored form below, block-cooperative: a thread block owns one (h, Delta) block tile and
- *           a chunk of k-points; the WD + WH exponentials per (k, band) are computed once per block and shared
- *           through shared memory; every thread keeps a TH x TD register tile of running products over all k of
- *           the chunk (no cross-thread reduction).  Falls back to FACTORED when the grid is much smaller than a
- *           block tile (e.g. a single h value) unless a shape is forced with fe_set_coop_shape.
- * FACTORED: per-thread version.  Uses 2cosh(d/T) + 2cosh(R/T) = B(h) + A(Delta): per (k, band) TH + TD exponentials in
- *           extended range (fp64 mantissa + int exponent), per term one add and one multiply into a running
- *           product; the logarithm is taken once per thread at the end.
- * DIRECT  : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5
- *           (the stable form max(R,|d|) + T ln(1 + u + v + uv)).
- * WINDOWED: DIRECT, but a term whose thermal part is below half an ulp of its T=0 part (|R-|d|| >= 37 T) adds
- *           only max(R,|d|); the decision is taken per warp.  Bit-identical to DIRECT.                      */
-#define FE_EVAL_FACTORED 0
-#define FE_EVAL_DIRECT   1
-#define FE_EVAL_WINDOWED 2
+/* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); both compute the same sums ----
+ * COOP_EO : default.  The block-cooperative factored kernel with a block-uniform early-out: a (k, band) slot whose
+ *           2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^58 over a whole group of h values contributes
+ *           T ln Z_ij = R_j (exact to fp64), so it needs no pair products; the other slots are compacted and run
+ *           through the dense pipeline.  Same results to ~1e-15 relative; several times fewer FP64 instructions
+ *           at low T.
+ * COOP    : the dense variant (every pair of every slot is multiplied out).  Uses 2cosh(d/T) + 2cosh(R/T) =
+ *           B(h) + A(Delta): a thread block owns one (h, Delta) block tile and a chunk of k-points; the exponentials
+ *           per (k, band) are computed once per block and shared through shared memory; every thread keeps a register
+ *           tile of running products over all k of the chunk (no cross-thread reduction).
+ * Three further formulations of the same sums (per-thread factored, direct Eq. 4 / Eq. 5 per term, windowed) are kept
+ * as cross-checks for the tests; their selectors are in fe_debug.h.                                           */
 #define FE_EVAL_COOP     3
 #define FE_EVAL_COOP_EO  4
 
@@ -98,7 +90,8 @@ int fe_create(const fe_model_params* params, int32_t N, double T, fe_handle** ou
 /* Change T (> 0, finite) for subsequent calls (config 4 scans two temperatures).  Host-only, cheap. */
 int fe_set_temperature(fe_handle* h, double T);
 
-/* Select FE_EVAL_COOP_EO (default), FE_EVAL_COOP, FE_EVAL_FACTORED, FE_EVAL_DIRECT or FE_EVAL_WINDOWED for subsequent fe_omega_grid calls. */
+/* Select FE_EVAL_COOP_EO (default) or FE_EVAL_COOP (or one of the cross-check modes of fe_debug.h) for subsequent
+ * fe_omega_grid calls.  Unknown mode: FE_EINVAL. */
 int fe_set_eval_mode(fe_handle* h, int32_t mode);
 
 /* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,
@@ -196,30 +189,11 @@ int fe_get_last_launch_info(fe_handle* h, int32_t* info6);
 /* Number of kernel launches this handle has issued since creation (all kernels of this library). */
 int fe_get_launch_count(fe_handle* h, int64_t* launches);
 
-/* Tuning knobs (optional).  tile: 0 = auto, else index into the built-in tile table (see fe_tile_info);
- * target_blocks: minimum number of thread blocks K1 should be split into (0 = auto).               */
-int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks);
-int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past the end of the table */
-/* FE_EVAL_COOP block shape: 0 = auto, else index (from 1) into the built-in shape table; forcing a shape also
- * disables the fallback to FE_EVAL_FACTORED.  fe_coop_shape_info: info6 = {TH, TD, WH, WD, threads per block,
- * resident blocks per SM}; FE_EINVAL past the end of the table. */
-int fe_set_coop_shape(fe_handle* h, int32_t shape);
-int fe_coop_shape_info(int32_t shape, int32_t* info6);
-/* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP(_EO): bit 0 = always take the robust per-pair path (this also switches
- * the early-out of FE_EVAL_COOP_EO off), bit 1 = never use the per-tile h recurrence (FACTORED).  Results are the same
- * sums; only the code path changes (lets tests cover each path).                                            */
-int fe_set_debug_flags(fe_handle* h, int32_t flags);
-
 /* FP64 DFMA-chain microbenchmark on the current device (register-resident, no memory traffic):
  * runs `blocks` blocks of 256 threads, each thread `iters` x 16 dependent-chain-interleaved DFMAs,
  * and returns elapsed ms and the number of DFMA instructions (thread-level) executed.
  * Used to measure the FP64 roofline denominator in the same run as the benchmark.                  */
 int fe_fp64_peak_probe(int32_t blocks, int32_t iters, float* ms, double* dfma_count, void* cuda_stream);
-
-/* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
- * y[i] = exp(x[i]) for x <= 0 (which = 0) or ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the k-sum
- * kernel evaluates the thermal term of Eq. 5.  Lets tests check it in isolation.       */
-int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream);
 
 void fe_destroy(fe_handle* h);          /* frees all device/host scratch; NULL is a no-op */
 const char* fe_strerror(int code);      /* static or thread-local string; never NULL      */

@@ -1,0 +1,50 @@
+/*
+ * fe_debug.h -- test and tuning hooks of libfe.  NOT part of the boundary SURVEY.md 8(b) lists (that is include/fe.h):
+ * included only by the tests, bench.py's binding and the library itself.  Same conventions as fe.h (C ABI, int error
+ * codes, fe_strerror).  Nothing here changes WHAT is computed, only which kernel formulation / launch shape computes it.
+ */
+#ifndef FE_DEBUG_H_
+#define FE_DEBUG_H_
+
+#include "fe.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- cross-check formulations of the k-sum (fe_set_eval_mode); same sums as FE_EVAL_COOP (Eq. 4 / Eq. 5) ----
+ * FACTORED: per-thread version of the factored form.  Per (k, band) TH + TD exponentials in extended range (fp64
+ *           mantissa + int exponent), per term one add and one multiply into a running product; the logarithm is
+ *           taken once per thread at the end.  fe_omega_grid falls back to it when the (h, Delta) grid is much smaller
+ *           than a block tile of FE_EVAL_COOP (e.g. a single h value) unless a shape is forced with fe_set_coop_shape.
+ * DIRECT  : every (k, band, q, h, Delta) term evaluates both exponentials and the logarithm of Eq. 5
+ *           (the stable form max(R,|d|) + T ln(1 + u + v + uv)).
+ * WINDOWED: DIRECT, but a term whose thermal part is below half an ulp of its T=0 part (|R-|d|| >= 37 T) adds
+ *           only max(R,|d|); the decision is taken per warp.  Bit-identical to DIRECT.                      */
+#define FE_EVAL_FACTORED 0
+#define FE_EVAL_DIRECT   1
+#define FE_EVAL_WINDOWED 2
+
+/* Tuning knobs (optional).  tile: 0 = auto, else index into the built-in tile table (see fe_tile_info);
+ * target_blocks: minimum number of thread blocks K1 should be split into (0 = auto).               */
+int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks);
+int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past the end of the table */
+/* FE_EVAL_COOP block shape: 0 = auto, else index (from 1) into the built-in shape table; forcing a shape also
+ * disables the fallback to FE_EVAL_FACTORED.  fe_coop_shape_info: info6 = {TH, TD, WH, WD, threads per block,
+ * resident blocks per SM}; FE_EINVAL past the end of the table. */
+int fe_set_coop_shape(fe_handle* h, int32_t shape);
+int fe_coop_shape_info(int32_t shape, int32_t* info6);
+/* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP(_EO): bit 0 = always take the robust per-pair path (this also switches
+ * the early-out of FE_EVAL_COOP_EO off), bit 1 = never use the per-tile h recurrence (FACTORED).  Results are the same
+ * sums; only the code path changes (lets tests cover each path).                                            */
+int fe_set_debug_flags(fe_handle* h, int32_t flags);
+
+/* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
+ * y[i] = exp(x[i]) for x <= 0 (which = 0) or ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the k-sum
+ * kernel evaluates the thermal term of Eq. 5.  Lets tests check it in isolation.       */
+int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FE_DEBUG_H_ */

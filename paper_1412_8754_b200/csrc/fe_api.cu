@@ -8,6 +8,7 @@
 #include <new>
 
 #include "../../include/fe.h"
+#include "../../include/fe_debug.h"
 #define FE_PLAIN_KERNELS
 #include "fe_kernels.cuh"
 #include "fe_bands3.cuh"
@@ -42,6 +43,7 @@ constexpr CoopShape kCoopShapes[] = {{16, 4, 4, 4, 4, 2}, {16, 4, 1, 4, 2, 2}, {
 constexpr int kNumCoopShapes = sizeof(kCoopShapes) / sizeof(kCoopShapes[0]);
 constexpr int kStageSlots = 4;
 constexpr int kSChunksMax = 128;
+constexpr int kMaxQ = 65534;   // q sits on gridDim.y (<= 65535) of KS / KB; KB adds one row for the unshifted table
 
 struct StageSlot {
   double* host = nullptr;    // pinned
@@ -286,6 +288,7 @@ int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh
   if (!q_xy || !h_list || !delta) { snprintf(g_errbuf, sizeof g_errbuf, "a list pointer is NULL"); return FE_EINVAL; }
   if (nq < 1 || nh < 1 || nd < 1) { snprintf(g_errbuf, sizeof g_errbuf, "nq, nh, nd must be >= 1"); return FE_EINVAL; }
   if ((double)nq * nh * nd > 2.0e9) { snprintf(g_errbuf, sizeof g_errbuf, "grid too large (nq*nh*nd > 2e9)"); return FE_EINVAL; }
+  if (nq > kMaxQ) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be <= %d (q is a grid dimension of the table kernels)", kMaxQ); return FE_EINVAL; }
   for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
   for (int i = 0; i < nh; ++i) if (!isfinite(h_list[i])) { snprintf(g_errbuf, sizeof g_errbuf, "h[%d] not finite", i); return FE_EINVAL; }
   for (int i = 0; i < nd; ++i) if (!isfinite(delta[i])) { snprintf(g_errbuf, sizeof g_errbuf, "delta[%d] not finite", i); return FE_EINVAL; }
@@ -293,9 +296,20 @@ int check_lists(const double* q_xy, int32_t nq, const double* h_list, int32_t nh
 }
 
 // sp: 0 = the handle's fp64 evaluation mode; 1 = K1s SP; 2 = K1s SPFM (fe_ksum_sp.cuh)
+int check_device(const fe_handle* h) {
+  int dev = -1;
+  FE_CUDA(cudaGetDevice(&dev));
+  if (dev != h->device) {
+    snprintf(g_errbuf, sizeof g_errbuf, "handle was created on device %d but device %d is current", h->device, dev);
+    return FE_EINVAL;
+  }
+  return FE_OK;
+}
+
 int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                     const double* delta, int32_t nd, double* omega_dev, cudaStream_t st, int sp = 0) {
   const int N = h->N;
+  if (int rcd = check_device(h)) return rcd;
   // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
   int mode = h->mode;
   if (sp) {
@@ -683,10 +697,11 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
 
 int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
   if (!h || !q_xy || !chi_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle, q_xy or chi_dev is NULL"); return FE_EINVAL; }
-  if (nq < 1 || nq > 65535 || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, 65535], hz finite"); return FE_EINVAL; }
+  if (nq < 1 || nq > kMaxQ || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, %d], hz finite", kMaxQ); return FE_EINVAL; }
   for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = h->N, nb = h->nb, nbb = nb * nb;
+  if (int rcd = check_device(h)) return rcd;
   double *hs, *ds; StageSlot* slot;
   int rc = stage_lists(h, (size_t)3 * nq, st, &hs, &ds, &slot);
   if (rc) return rc;
@@ -797,7 +812,12 @@ int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double*
   if ((rc = omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, h->d_omega, st, 1 + fast_math))) return rc;
   // 2. candidates
   FE_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * (size_t)nd, st));
-  fe_mark_candidates_kernel<<<(ncol + 7) / 8, 256, 0, st>>>(ncol, nd, margin_rel, h->d_omega, h->d_flags);
+  // the low-precision error scales with the magnitude of the summed terms (~ N^2 (band half-width + |mu|) per band),
+  // not with |Omega_min|, which can be close to zero: the margin is relative to the larger of the two
+  int nbm = 0;
+  for (int e = 0; e < h->nb; ++e) nbm += (h->p.band_mask >> e) & 1;
+  const double abs_scale = (double)h->N * (double)h->N * nbm * (band_half_width(h->p) + fabs(h->p.mu));
+  fe_mark_candidates_kernel<<<(ncol + 7) / 8, 256, 0, st>>>(ncol, nd, margin_rel, abs_scale, h->d_omega, h->d_flags);
   FE_CUDA(cudaGetLastError());
   h->launches++;
   FE_CUDA(cudaMemcpyAsync(h->h_flags, h->d_flags, sizeof(int32_t) * (size_t)nd, cudaMemcpyDeviceToHost, st));

@@ -706,11 +706,12 @@ __global__ void __launch_bounds__(256) fe_argmin_q_kernel(int nq, int nh, int nd
 // ---------------------------------------------------------------------------------------------------
 // K5 / K6 (fe_scan_verified: "run larger parameter scans at lower precision and then selectively verify with double
 // precision calculations").  K5: one warp per (q, h) column of the low-precision Omega: every Delta
-// index whose value is within margin_rel |min| of the column minimum is flagged (all writers store 1: benign).
+// index whose value is within margin_rel max(|min|, abs_scale) of the column minimum is flagged (all writers store 1:
+// benign); abs_scale = N^2 (#bands) (band half-width + |mu|) bounds the magnitude of the sums the rounding acts on.
 // K6: column minima found on the reduced (verified) Delta list are mapped back to indices of the full list.
 // ---------------------------------------------------------------------------------------------------
-__global__ void fe_mark_candidates_kernel(int ncol, int nd, double margin_rel, const double* __restrict__ omega,
-                                          int32_t* __restrict__ flags) {
+__global__ void fe_mark_candidates_kernel(int ncol, int nd, double margin_rel, double abs_scale,
+                                          const double* __restrict__ omega, int32_t* __restrict__ flags) {
   const int col = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (col >= ncol) return;
   const int lane = threadIdx.x & 31;
@@ -719,7 +720,7 @@ __global__ void fe_mark_candidates_kernel(int ncol, int nd, double margin_rel, c
   for (int i = lane; i < nd; i += 32) best = fmin(best, om[i]);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
-  const double thr = best + margin_rel * fabs(best);
+  const double thr = best + margin_rel * fmax(fabs(best), abs_scale);
   for (int i = lane; i < nd; i += 32)
     if (om[i] <= thr) flags[i] = 1;
 }

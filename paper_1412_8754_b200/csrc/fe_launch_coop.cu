@@ -1,6 +1,7 @@
 // fe_launch_coop.cu -- K1c instantiations of ONE block shape.  Compiled once per shape by build.py with
 // -DFE_COOP_ID=i -DFE_COOP_TH=.. -DFE_COOP_TD=.. -DFE_COOP_LH=.. -DFE_COOP_NW=.. -DFE_COOP_KB=.. -DFE_COOP_MINB=..
 #include "../../include/fe.h"
+#include "../../include/fe_debug.h"
 #include "fe_launch.h"
 
 namespace fe {
@@ -10,12 +11,10 @@ template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
 cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
   using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
   auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB>;
-  static bool attr_set = false;     // per instantiation; the attribute is sticky for the function
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // The opt-in is per DEVICE (and a handle binds to the device current at fe_create), so it is set before every
+  // launch: a host-side call of a few hundred nanoseconds, no static state shared between devices or host threads.
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+  if (e != cudaSuccess) return e;
   kern<<<grid, G::NT, G::smem_bytes, st>>>(P);
   return cudaGetLastError();
 }

@@ -1,6 +1,7 @@
 // fe_launch_tile.cu -- K1 (direct / windowed) and K1f (factored) instantiations of ONE register tile.
 // Compiled once per tile by build.py with -DFE_TILE_ID=i -DFE_TILE_TH=.. -DFE_TILE_TD=..
 #include "../../include/fe.h"
+#include "../../include/fe_debug.h"
 #include "fe_launch.h"
 
 namespace fe {

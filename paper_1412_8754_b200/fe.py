@@ -16,9 +16,12 @@ from . import build as _build
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_EARCH = 0, -1, -2, -3, -4
 EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3, 4
 
-EXPORTS = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility", "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host",
-           "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info", "fe_get_launch_count", "fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info",
-           "fe_fp64_peak_probe", "fe_debug_math", "fe_destroy", "fe_strerror"]
+# include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
+EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
+               "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
+               "fe_get_launch_count", "fe_fp64_peak_probe", "fe_destroy", "fe_strerror"]
+EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math"]
+EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
 
 class FeError(RuntimeError):

@@ -2,8 +2,9 @@
 
 Calls ONLY oracle/ (never the CUDA path).  The GPU parity tests at full size (configs 3-5) compare against
 these stored values so that the GPU box does not spend minutes of host time re-deriving them; the samples are
-whole (q, h) columns for configs 3-4 (so the argmin check is meaningful) and strided Delta subsets of columns
-for config 5.  Floats are stored with repr() (exact round trip).
+WHOLE (q, h) columns (all Delta, full k-sum), so the argmin check against the oracle is meaningful: 12 columns of
+config 3, 16 per temperature of config 4, 4 per seed for seeds 1-3 of config 5 (each seed is its own
+run with its own perturbed hoppings, stored with the run).  Floats are stored with repr() (exact round trip).
 
     python tests/golden/make_golden.py [3 4 5]
 """
@@ -22,11 +23,12 @@ from paper_1412_8754_b200 import workloads as W      # noqa: E402
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 
-PLAN = {            # cfg: (number of (q,h) columns, Delta indices per column or None = all)
+PLAN = {            # cfg: (number of (q,h) columns per run, Delta indices per column or None = all)
     3: (12, None),
-    4: (4, None),
-    5: (3, 24),
+    4: (16, None),
+    5: (4, None),
 }
+SEEDS = {5: (1, 2, 3)}      # config 5: "seed-generated random perturbation of hoppings ... per run" (BASELINE.json)
 
 
 def delta_subset(nd, n):
@@ -38,21 +40,27 @@ def delta_subset(nd, n):
 
 def main(cfgs):
     for c in cfgs:
-        w = W.config(c)
         ncol, nsub = PLAN[c]
-        cols = W.sample_columns(w, ncol, c)
-        ids = delta_subset(w.nd, nsub)
-        out = dict(config=c, workload=w.name, N=w.N, params=w.params, oracle="oracle/fe_oracle.c feo_omega_column",
+        w0 = W.config(c)
+        out = dict(config=c, workload=w0.name, N=w0.N, params=w0.params, oracle="oracle/fe_oracle.c feo_omega_column",
                    generated_by="tests/golden/make_golden.py", runs=[])
-        for T in w.T:
-            t0 = time.time()
-            entries = []
-            for (iq, ih) in cols:
-                om = O.omega_column(w.params, w.N, T, w.q[iq], w.h[ih], w.delta[ids])
-                entries.append(dict(iq=iq, ih=ih, q=[repr(float(x)) for x in w.q[iq]], h=repr(float(w.h[ih])),
-                                    id=ids, omega=[repr(float(x)) for x in om]))
-                print(f"cfg{c} T={T} col ({iq},{ih}) done, {time.time() - t0:.1f}s", flush=True)
-            out["runs"].append(dict(T=T, columns=entries))
+        for seed in SEEDS.get(c, (None,)):
+            w = W.config(c) if seed is None else W.config(c, seed=seed)
+            # seed 1 / unseeded configs keep the column sample of the config id; other seeds draw their own
+            cols = W.sample_columns(w, ncol, c if seed in (None, 1) else c + 1000 * (seed - 1))
+            ids = delta_subset(w.nd, nsub)
+            for T in w.T:
+                t0 = time.time()
+                entries = []
+                for (iq, ih) in cols:
+                    om = O.omega_column(w.params, w.N, T, w.q[iq], w.h[ih], w.delta[ids])
+                    entries.append(dict(iq=iq, ih=ih, q=[repr(float(x)) for x in w.q[iq]], h=repr(float(w.h[ih])),
+                                        id=ids, omega=[repr(float(x)) for x in om]))
+                    print(f"cfg{c} seed={seed} T={T} col ({iq},{ih}) done, {time.time() - t0:.1f}s", flush=True)
+                run = dict(T=T, columns=entries)
+                if seed is not None:
+                    run.update(seed=seed, workload=w.name, params=w.params)
+                out["runs"].append(run)
         with open(os.path.join(HERE, f"oracle_cfg{c}.json"), "w") as f:
             json.dump(out, f, indent=0)
         print("wrote", f.name, flush=True)

@@ -389,6 +389,7 @@ def test_randomised_grids_all_models(fe, oracle):
     """Seeded random workloads (models, N odd / even, T over four decades, list lengths around the tile edges, q / h /
     Delta of both signs, band masks, k-splits): default mode and the dense variant against the oracle."""
     rng = np.random.default_rng(20141231)
+    n_small = n_total = 0
     for case in range(36):
         model = int(rng.choice([1, 2, 3]))
         N = int(rng.integers(5, 72))
@@ -412,36 +413,47 @@ def test_randomised_grids_all_models(fe, oracle):
                        np.sort(rng.uniform(-0.3 * hs, hs, size=nh)), np.sort(rng.uniform(-0.2 * ds, ds, size=nd)))
         tb = int(rng.choice([0, 0, 1, 300]))
         ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
-        # With a single, nearly empty band selected Omega(Delta) passes through zero along a column (the k-sum and the
-        # condensation term cancel), so the error is measured against the column's scale max_Delta |Omega|: that is
-        # the magnitude of the sums whose rounding the 1e-12 bound is about.
+        # The bound is elementwise, |dOmega| <= 1e-12 |Omega|.  Only where Omega(Delta) passes through zero along a column
+        # (a single, nearly empty band selected by band_mask: the k-sum and the condensation term cancel) is the
+        # elementwise ratio meaningless; elements with |Omega| < 1e-3 max_Delta |Omega| are measured against the
+        # column's scale instead, and fewer than 1 % of all elements may take that branch.
         scale = np.abs(ref).max(axis=-1, keepdims=True)
+        small = np.abs(ref) < 1e-3 * scale
+        n_small += int(small.sum())
+        n_total += ref.size
+        denom = np.where(small, scale, np.abs(ref))
         for mode in (None, fe.EVAL_COOP):
             om, idx, ds, os_ = run_gpu(fe, w, T, mode=mode, target_blocks=tb)
-            err = float(np.max(np.abs(om - ref) / scale))
+            err = float(np.max(np.abs(om - ref) / denom))
             assert err < RTOL, f"{w.name} mode={mode} T={T}: {err:.3e}"
             assert np.array_equal(idx, np.argmin(om, axis=-1).astype(np.int32)) and np.array_equal(os_, om.min(axis=-1))
+    assert n_small < 0.01 * n_total, (n_small, n_total)
 
 
 def test_full_size_properties_in_bench_launch_configuration(fe):
-    """Whole config-3 and config-4 steps exactly as bench.py launches them (all q, all h, all Delta in one call):
-    properties that hold at any size -- Omega(q) = Omega(-q) (O4), the early-out and the dense variant agree, the
-    on-device minima are the minima of the device Omega, reruns are bit-identical."""
+    """Whole config-3, config-4 and config-5 steps exactly as bench.py launches them (all q, all h, all Delta in one
+    call): properties that hold at any size -- Omega(q) = Omega(-q) (O4), the early-out and the dense variant agree, the
+    on-device minima are the minima of the device Omega, reruns are bit-identical (config 5: "fp64 with fixed-order
+    reduction" at N = 4096)."""
     import torch
-    for cfg, T in ((3, 0.001), (4, 0.01)):
+    for cfg, T in ((3, 0.001), (4, 0.01), (5, 0.0005)):
         w = W.config(cfg)
         with fe.FreeEnergy(w.params, w.N, T) as F:
             a = F.omega_grid(w.q, w.h, w.delta)
             idx, ds, os_ = F.argmin(a, w.delta)
             a2 = F.omega_grid(w.q, w.h, w.delta)
             b = F.omega_grid(-w.q, w.h, w.delta)
+            assert F.last_launch_info()["mode"] == fe.EVAL_COOP_EO
             F.set_eval_mode(fe.EVAL_COOP)
             c = F.omega_grid(w.q, w.h, w.delta)
+            c2 = F.omega_grid(w.q, w.h, w.delta)
+            assert F.last_launch_info()["mode"] == fe.EVAL_COOP
             torch.cuda.synchronize()
-            assert torch.equal(a, a2)
+            assert torch.equal(a, a2) and torch.equal(c, c2)
             assert float(((a - b).abs() / a.abs()).max()) < 1e-12
             assert float(((a - c).abs() / a.abs()).max()) < 1e-13
             assert torch.equal(os_, a.min(dim=-1).values) and torch.equal(idx.long(), a.argmin(dim=-1))
+            assert torch.equal(ds, torch.from_numpy(w.delta).cuda()[idx.long()])
             assert bool(torch.isfinite(a).all())
 
 
@@ -607,39 +619,54 @@ def load_golden(cfg):
     return json.load(open(path))
 
 
+def _golden_runs(cfg):
+    """(workload, T, columns) per stored run; config 5 stores one run per seed with that seed's perturbed hoppings."""
+    g = load_golden(cfg)
+    same = lambda a, b: {k: v for k, v in a.items() if k != "tb3"} == \
+        {k: (tuple(v) if isinstance(v, list) else v) for k, v in b.items() if k != "tb3"}      # noqa: E731
+    out = []
+    for run in g["runs"]:
+        w = W.config(cfg, seed=run["seed"]) if "seed" in run else W.config(cfg)
+        assert same(w.params, run.get("params", g["params"])), "stored parameters differ from workloads.config"
+        assert not any(w.params["tb3"])
+        out.append((w, run["T"], run["columns"]))
+    return out
+
+
 @pytest.mark.parametrize("mode", [4, 3, 0])
 @pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_full_size_configs_sampled_parity(fe, cfg, mode):
+    """Whole oracle (q, h) columns (all Delta, full k-sum) of configs 3-5 -- 12 / 16 per T / 4 per seed for seeds 1-3 --
+    against the device in the launch configuration bench.py times: Omega elementwise at 1e-12 and the per-column minimum
+    (index, Delta*, Omega*) against the oracle's (reading G11 for near-ties)."""
     import torch
-    g = load_golden(cfg)
-    w = W.config(cfg)
-    # (the stored files predate the three-band field `tb3`, which configs 3-5 do not use)
-    assert {k: v for k, v in w.params.items() if k != "tb3"} == \
-        {k: (tuple(v) if isinstance(v, list) else v) for k, v in g["params"].items() if k != "tb3"}
-    assert not any(w.params["tb3"])
-    for run in g["runs"]:
-        T = run["T"]
-        cols = run["columns"]
+    runs = _golden_runs(cfg)
+    if cfg == 5:
+        assert sorted(w.extra["seed"] for w, _, _ in runs) == [1, 2, 3]
+    if cfg == 5 and mode == 0:
+        runs = runs[:1]                 # the per-thread factored kernel is 4x slower: one seed is enough for it
+    n_exact = n_cols = 0
+    for w, T, cols in runs:
         iqs = sorted(set(c["iq"] for c in cols))
         with fe.FreeEnergy(w.params, w.N, T) as F:
             F.set_eval_mode(mode)
             for iq in iqs:
-                # the launch configuration bench.py times: one q, the full (h, Delta) grid of the config
+                # the launch configuration bench.py times: the full (h, Delta) grid of the config
                 om = F.omega_grid(w.q[iq:iq + 1], w.h, w.delta)
                 idx, ds, os_ = F.argmin(om, w.delta)
                 torch.cuda.synchronize()
+                assert F.last_launch_info()["mode"] == mode
                 om = om.cpu().numpy()[0]
-                idx = idx.cpu().numpy()[0]
+                idx, ds, os_ = idx.cpu().numpy()[0], ds.cpu().numpy()[0], os_.cpu().numpy()[0]
                 assert np.array_equal(idx, np.argmin(om, axis=-1).astype(np.int32))
-                assert np.array_equal(os_.cpu().numpy()[0], om.min(axis=-1))
+                assert np.array_equal(os_, om.min(axis=-1))
                 for c in (c for c in cols if c["iq"] == iq):
-                    ids = np.array(c["id"])
+                    ih = c["ih"]
+                    assert c["id"] == list(range(w.nd)), "golden columns must be whole columns"
                     ref = np.array([float(x) for x in c["omega"]])
-                    got = om[c["ih"], ids]
-                    err = max_rel(got, ref)
-                    assert err < RTOL, f"cfg{cfg} T={T} col ({iq},{c['ih']}): {err:.3e}"
-                    if len(ids) == w.nd:            # whole column stored: check the minimum against the oracle's
-                        check_argmin(ref[None, :], w.delta, idx[c["ih"]:c["ih"] + 1],
-                                     ds.cpu().numpy()[0, c["ih"]:c["ih"] + 1], os_.cpu().numpy()[0, c["ih"]:c["ih"] + 1])
-                    else:                           # sampled column: the device minimum may not lie above a sampled oracle value
-                        assert om[c["ih"]].min() <= ref.min() * (1 - RTOL) + 0 or om[c["ih"]].min() <= ref.min() + abs(ref.min()) * RTOL
+                    err = max_rel(om[ih], ref)
+                    assert err < RTOL, f"cfg{cfg} {w.name} T={T} col ({iq},{ih}): {err:.3e}"
+                    n_exact += check_argmin(ref[None, :], w.delta, idx[ih:ih + 1], ds[ih:ih + 1], os_[ih:ih + 1])
+                    n_cols += 1
+    assert n_cols == {3: 12, 4: 32, 5: 12 if mode else 4}[cfg]
+    assert n_exact >= n_cols // 2          # most stored columns have a resolved minimum (index compared bit-exactly)
