@@ -195,6 +195,11 @@ int fe_get_launch_count(fe_handle* h, int64_t* launches);
  * Used to measure the FP64 roofline denominator in the same run as the benchmark.                  */
 int fe_fp64_peak_probe(int32_t blocks, int32_t iters, float* ms, double* dfma_count, void* cuda_stream);
 
+/* First 16 hex digits of the sha256 of the kernel sources this library was compiled from (comments and white space
+ * removed; paper_1412_8754_b200/build.py source_hash).  bench.py uses it to tell whether committed profiler counts
+ * describe the kernels that are running.  Static string, never NULL. */
+const char* fe_build_source_hash(void);
+
 void fe_destroy(fe_handle* h);          /* frees all device/host scratch; NULL is a no-op */
 const char* fe_strerror(int code);      /* static or thread-local string; never NULL      */
 

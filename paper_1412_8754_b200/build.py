@@ -36,9 +36,30 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-Wno-deprecated-gpu-targets"]
 
 
+def source_hash() -> str:
+    """sha256 (first 16 hex digits) of the kernel sources as compiled: every file of csrc/ and include/, comments and
+    white space removed, so that only a change of code changes it.  bench.py compares it with the hash recorded beside
+    each committed ncu capture (profiles/COUNTS.md) before it uses that capture's instruction counts, and with the hash
+    compiled into libfe.so (fe_build_source_hash) before it trusts the library to be built from these sources."""
+    import hashlib
+    import re
+    files = sorted([os.path.join(CSRC, f) for f in os.listdir(CSRC)] +
+                   [os.path.join(ROOT, "include", f) for f in os.listdir(os.path.join(ROOT, "include"))])
+    hsh = hashlib.sha256()
+    for f in files:
+        if not f.endswith((".cu", ".cuh", ".h")):
+            continue
+        text = open(f).read()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+        text = re.sub(r"//[^\n]*", " ", text)
+        text = " ".join(text.split())
+        hsh.update(os.path.basename(f).encode() + b"\0" + text.encode() + b"\0")
+    return hsh.hexdigest()[:16]
+
+
 def units():
     """[(object name, source, extra -D flags)]"""
-    u = [("fe_api.o", "fe_api.cu", [])]
+    u = [("fe_api.o", "fe_api.cu", [f'-DFE_SOURCE_HASH="{source_hash()}"'])]
     for i, (th, td) in enumerate(TILES):
         u.append((f"fe_tile{i}.o", "fe_launch_tile.cu", [f"-DFE_TILE_ID={i}", f"-DFE_TILE_TH={th}", f"-DFE_TILE_TD={td}"]))
     for i, s in enumerate(COOP_SHAPES):

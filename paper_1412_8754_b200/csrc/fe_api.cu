@@ -958,6 +958,11 @@ void fe_destroy(fe_handle* h) {
   delete h;
 }
 
+#ifndef FE_SOURCE_HASH
+#define FE_SOURCE_HASH "unknown"
+#endif
+const char* fe_build_source_hash(void) { return FE_SOURCE_HASH; }
+
 const char* fe_strerror(int code) {
   switch (code) {
     case FE_OK: return "ok";

@@ -19,7 +19,7 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 # include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
-               "fe_get_launch_count", "fe_fp64_peak_probe", "fe_destroy", "fe_strerror"]
+               "fe_get_launch_count", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
@@ -84,11 +84,23 @@ def lib():
     L.fe_destroy.restype = None
     L.fe_strerror.argtypes = [C.c_int]
     L.fe_strerror.restype = C.c_char_p
+    L.fe_build_source_hash.argtypes = []
+    L.fe_build_source_hash.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("fe_destroy", "fe_strerror"):
+        if name not in ("fe_destroy", "fe_strerror", "fe_build_source_hash"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
+
+
+def built_source_hash() -> str:
+    """Hash of the kernel sources libfe.so was compiled from (fe_build_source_hash)."""
+    return lib().fe_build_source_hash().decode()
+
+
+def source_hash() -> str:
+    """Hash of the kernel sources in the tree now (build.source_hash)."""
+    return _build.source_hash()
 
 
 def _check(rc):
@@ -273,9 +285,12 @@ class FreeEnergy:
                                       int(bool(fast_math)), C.c_void_p(out.data_ptr()), _stream(stream)))
         return out
 
-    def scan_verified(self, q, h, delta, fast_math=False, margin_rel=1e-5, stream=None):
-        """Single-precision screening + fp64 verification of the candidates: (idx, delta*, omega*, n_verified)."""
+    def scan_verified(self, q, h, delta, fast_math=False, margin_rel=1e-5, stream=None, screen=None):
+        """Low-precision screening + fp64 verification of the candidates: (idx, delta*, omega*, n_verified).
+        screen: "sp" | "spfm" (the paper's single-precision builds) -- overrides fast_math when given."""
         import torch
+        if screen is not None:
+            fast_math = {"sp": 0, "spfm": 1}[screen]
         q, h, d = _f64(q).reshape(-1, 2), _f64(h), _f64(delta)
         shp = (q.shape[0], h.shape[0])
         idx = torch.empty(shp, dtype=torch.int32, device="cuda")
