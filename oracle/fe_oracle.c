@@ -274,6 +274,62 @@ int feo_omega_column(const feo_params* p, int32_t N, double T, double qx, double
     return 0;
 }
 
+/*
+ * Diagnostic for the parity tests (not a step of the method): the MAGNITUDE of the sum feo_omega_column forms,
+ *   mag_out[id] = sum_{eps, k} ( |f(E+)| + |f(E-)| + |C_{eps k}| ) + |condensation term|,
+ * i.e. the same terms of Eq. 5 with absolute values.  mag / |Omega| is the condition number of the
+ * k-sum: where the terms cancel (a single, nearly empty band selected by band_mask) no fp64 evaluation can be
+ * accurate to 1e-12 of |Omega| itself, and the tests bound the error by the rounding of the terms instead.
+ */
+int feo_omega_column_magnitude(const feo_params* p, int32_t N, double T, double qx, double qy, double h,
+                               const double* delta, int32_t nd, double* mag_out) {
+    if (!p || !delta || !mag_out || N < 1 || nd < 1 || !(T > 0.0) || !(p->U > 0.0)) return -1;
+    if (p->model != 1 && p->model != 2 && p->model != 3) return -1;
+    const int nb = feo_num_bands(p);
+    const size_t nk = (size_t)N * (size_t)N;
+    double* up  = (double*)malloc(sizeof(double) * nk * nb);
+    double* dn  = (double*)malloc(sizeof(double) * nk * nb);
+    double* cst = (double*)malloc(sizeof(double) * nk * nb);
+    double* eta = (double*)malloc(sizeof(double) * nk);
+    if (!up || !dn || !cst || !eta) { free(up); free(dn); free(cst); free(eta); return -2; }
+#pragma omp parallel for schedule(static)
+    for (int32_t j = 0; j < N; ++j)
+        for (int32_t i = 0; i < N; ++i) {
+            const double kx = 2.0 * M_PI * (double)i / (double)N;
+            const double ky = 2.0 * M_PI * (double)j / (double)N;
+            double Ek[3], Ekq[3];
+            feo_band_energies(p, kx, ky, Ek);
+            feo_band_energies(p, -kx + qx, -ky + qy, Ekq);
+            const size_t k = (size_t)j * N + i;
+            eta[k] = feo_eta(p, kx, ky);
+            for (int e = 0; e < nb; ++e) {
+                up[e * nk + k]  = Ek[e]  - p->mu - h;
+                dn[e * nk + k]  = Ekq[e] - p->mu + h;
+                cst[e * nk + k] = (p->const_mode == 0) ? dn[e * nk + k] : (Ek[e] - p->mu + h);
+            }
+        }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t id = 0; id < nd; ++id) {
+        const double D = delta[id];
+        feo_acc A = {0.0L, 0.0L};
+        for (int e = 0; e < nb; ++e) {
+            if (!((p->band_mask >> e) & 1)) continue;
+            for (size_t k = 0; k < nk; ++k) {
+                double Ep, Em;
+                feo_quasiparticle(up[e * nk + k], dn[e * nk + k], D * eta[k], &Ep, &Em);
+                acc_add(&A, fabsl((long double)feo_thermal(Ep, T)));
+                acc_add(&A, fabsl((long double)feo_thermal(Em, T)));
+                acc_add(&A, fabsl((long double)cst[e * nk + k]));
+            }
+        }
+        acc_add(&A, fabsl((long double)p->cond_mult * (long double)nk * (long double)D * (long double)D
+                          / (long double)p->U));
+        mag_out[id] = (double)(A.s + A.c);
+    }
+    free(up); free(dn); free(cst); free(eta);
+    return 0;
+}
+
 /* Whole grid, Algorithm 1's outer loops: q, then h, then the column above.
  * omega_out index (iq*nh + ih)*nd + id  (Delta fastest).                                      */
 int feo_omega_grid(const feo_params* p, int32_t N, double T,

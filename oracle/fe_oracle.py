@@ -49,6 +49,8 @@ def lib():
         L.feo_omega_column.argtypes = [pp, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                        dp, C.c_int32, dp]
         L.feo_omega_column.restype = C.c_int
+        L.feo_omega_column_magnitude.argtypes = L.feo_omega_column.argtypes
+        L.feo_omega_column_magnitude.restype = C.c_int
         L.feo_omega_grid.argtypes = [pp, C.c_int32, C.c_double, dp, C.c_int32, dp, C.c_int32,
                                      dp, C.c_int32, dp]
         L.feo_omega_grid.restype = C.c_int
@@ -137,6 +139,25 @@ def omega_column(p: dict, N: int, T: float, q, h: float, delta) -> np.ndarray:
                                 _dptr(out))
     if rc:
         raise ValueError(f"feo_omega_column failed: {rc}")
+    return out
+
+
+def omega_grid_magnitude(p: dict, N: int, T: float, q, h, delta) -> np.ndarray:
+    """Sum of the ABSOLUTE values of the terms of Omega[iq, ih, id] (feo_omega_column_magnitude): the scale the rounding
+    of the k-sum acts on; magnitude / |Omega| is the condition number of the sum."""
+    sp = _params(p)
+    q = np.ascontiguousarray(q, dtype=np.float64).reshape(-1, 2)
+    h = np.ascontiguousarray(h, dtype=np.float64).reshape(-1)
+    d = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+    out = np.empty((q.shape[0], h.shape[0], d.shape[0]), dtype=np.float64)
+    for iq in range(q.shape[0]):
+        for ih in range(h.shape[0]):
+            col = np.empty(d.shape[0], dtype=np.float64)
+            rc = lib().feo_omega_column_magnitude(C.byref(sp), N, T, float(q[iq, 0]), float(q[iq, 1]), float(h[ih]),
+                                                  _dptr(d), d.shape[0], _dptr(col))
+            if rc:
+                raise ValueError(f"feo_omega_column_magnitude failed: {rc}")
+            out[iq, ih] = col
     return out
 
 

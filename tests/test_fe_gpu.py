@@ -389,7 +389,8 @@ def test_randomised_grids_all_models(fe, oracle):
     """Seeded random workloads (models, N odd / even, T over four decades, list lengths around the tile edges, q / h /
     Delta of both signs, band masks, k-splits): default mode and the dense variant against the oracle."""
     rng = np.random.default_rng(20141231)
-    n_small = n_total = 0
+    COND = 100.0
+    n_ill = n_total = 0
     for case in range(36):
         model = int(rng.choice([1, 2, 3]))
         N = int(rng.integers(5, 72))
@@ -413,21 +414,28 @@ def test_randomised_grids_all_models(fe, oracle):
                        np.sort(rng.uniform(-0.3 * hs, hs, size=nh)), np.sort(rng.uniform(-0.2 * ds, ds, size=nd)))
         tb = int(rng.choice([0, 0, 1, 300]))
         ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
-        # The bound is elementwise, |dOmega| <= 1e-12 |Omega|.  Only where Omega(Delta) passes through zero along a column
-        # (a single, nearly empty band selected by band_mask: the k-sum and the condensation term cancel) is the
-        # elementwise ratio meaningless; elements with |Omega| < 1e-3 max_Delta |Omega| are measured against the
-        # column's scale instead, and fewer than 1 % of all elements may take that branch.
-        scale = np.abs(ref).max(axis=-1, keepdims=True)
-        small = np.abs(ref) < 1e-3 * scale
-        n_small += int(small.sum())
-        n_total += ref.size
-        denom = np.where(small, scale, np.abs(ref))
+        # The bound is elementwise: |dOmega| <= 1e-12 |Omega|.  It cannot hold where the k-sum cancels: with a single,
+        # nearly empty band selected by band_mask, Omega = sum_k (f + f + C) + cond is orders of magnitude smaller
+        # than its terms (and passes through zero along a column), and ANY fp64 evaluation -- the oracle's own terms
+        # included -- carries the rounding of the terms, eps x sum |terms|.  The oracle reports that magnitude
+        # (feo_omega_column_magnitude).  An element may miss the elementwise bound only if its sum is conditioned worse
+        # than COND = 100 (magnitude > 100 |Omega|), it must then be within 1e-14 x magnitude (45 eps: the same
+        # arithmetic budget), and fewer than 1 % of all elements may take that branch.
+        mag = None
         for mode in (None, fe.EVAL_COOP):
             om, idx, ds, os_ = run_gpu(fe, w, T, mode=mode, target_blocks=tb)
-            err = float(np.max(np.abs(om - ref) / denom))
-            assert err < RTOL, f"{w.name} mode={mode} T={T}: {err:.3e}"
+            err = np.abs(om - ref)
+            miss = err > RTOL * np.abs(ref)
+            if miss.any():
+                if mag is None:
+                    mag = oracle.omega_grid_magnitude(w.params, w.N, T, w.q, w.h, w.delta)
+                assert np.all(mag[miss] > COND * np.abs(ref[miss])), \
+                    f"{w.name} mode={mode} T={T}: {float((err / np.abs(ref))[miss & (mag <= COND * np.abs(ref))].max()):.3e} on a well-conditioned element"
+                assert np.all(err[miss] <= (RTOL / COND) * mag[miss]), f"{w.name} mode={mode} T={T}: {float((err / mag)[miss].max()):.3e} of the magnitude"
+                n_ill += int(miss.sum())
+            n_total += ref.size
             assert np.array_equal(idx, np.argmin(om, axis=-1).astype(np.int32)) and np.array_equal(os_, om.min(axis=-1))
-    assert n_small < 0.01 * n_total, (n_small, n_total)
+    assert n_ill < 0.01 * n_total, (n_ill, n_total)
 
 
 def test_full_size_properties_in_bench_launch_configuration(fe):

@@ -532,3 +532,27 @@ def test_survey_anchor_config1(oracle):
     assert idx[0, 0] == 47
     assert abs(os_[0, 0] / w.N**2 - (-1.63885196927)) < 1e-10
     assert abs(om[0, 0, 0] / w.N**2 - (-1.61938750152)) < 1e-10
+
+
+def test_magnitude_diagnostic(oracle):
+    """feo_omega_column_magnitude (the scale the parity tests measure ill-conditioned sums against): triangle
+    inequality against Omega itself; for a completely filled band every term of Eq. 5 is negative, so the magnitude is
+    -Omega + 2 x condensation term exactly; in the atomic limit (t = 0) every k contributes the same closed-form term."""
+    d = np.array([0.0, 0.13, 0.4])
+    q, h = np.array([[0.3, -0.2]]), np.array([0.07])
+    for p in (W.model_params(), W.model_params(band_mask=1, cond_mult=1.0), W.model_params(model=W.MODEL_THREE_BAND, mu=W.THREE_BAND_MU, band_mask=4, cond_mult=1.0)):
+        om = oracle.omega_grid(p, 12, 0.01, q, h, d)
+        mag = oracle.omega_grid_magnitude(p, 12, 0.01, q, h, d)
+        assert np.all(mag >= np.abs(om) * (1 - 1e-14))
+    p = W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(1.0,), mu=9.0, U=2.0)      # filled band
+    om = oracle.omega_grid(p, 10, 0.02, q, h, d)[0, 0]
+    mag = oracle.omega_grid_magnitude(p, 10, 0.02, q, h, d)[0, 0]
+    cond = 1.0 * 100 * d * d / 2.0
+    assert np.allclose(mag, -om + 2 * cond, rtol=1e-13, atol=0)
+    p = W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(0.0,), mu=-0.3, U=2.0)     # atomic limit
+    T, hh = 0.05, 0.07
+    mag = oracle.omega_grid_magnitude(p, 6, T, q, np.array([hh]), d)[0, 0]
+    R = np.sqrt(0.3 ** 2 + d ** 2)
+    f = lambda x: -T * np.logaddexp(0.0, -x / T)        # noqa: E731
+    want = 36 * (np.abs(f(-hh + R)) + np.abs(f(-hh - R)) + abs(0.3 + hh)) + 36 * d * d / 2.0
+    assert np.allclose(mag, want, rtol=1e-13, atol=0)
