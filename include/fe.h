@@ -53,10 +53,10 @@ extern "C" {
 
 /* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); both compute the same sums ----
  * COOP_EO : default.  The block-cooperative factored kernel with a block-uniform early-out: a (k, band) slot whose
- *           2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^58 over a whole group of h values contributes
- *           T ln Z_ij = R_j (exact to fp64), so it needs no pair products; the other slots are compacted and run
- *           through the dense pipeline.  Same results to ~1e-15 relative; several times fewer FP64 instructions
- *           at low T.
+ *           2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^48 over the whole block tile contributes
+ *           T ln Z_ij = R_j (what is neglected is below half an ulp of the term), so it needs no pair products; the
+ *           other slots are compacted and run through the dense pipeline.  Same results to ~1e-15 relative; several
+ *           times fewer FP64 instructions at low T.
  * COOP    : the dense variant (every pair of every slot is multiplied out).  Uses 2cosh(d/T) + 2cosh(R/T) =
  *           B(h) + A(Delta): a thread block owns one (h, Delta) block tile and a chunk of k-points; the exponentials
  *           per (k, band) are computed once per block and shared through shared memory; every thread keeps a register

@@ -40,8 +40,9 @@ int fe_coop_shape_info(int32_t shape, int32_t* info6);
 int fe_set_debug_flags(fe_handle* h, int32_t flags);
 
 /* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
- * y[i] = exp(x[i]) for x <= 0 (which = 0) or ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the k-sum
- * kernel evaluates the thermal term of Eq. 5.  Lets tests check it in isolation.       */
+ * y[i] = exp(x[i]) for x <= 0 (which = 0), ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the direct k-sum
+ * kernel evaluates the thermal term of Eq. 5, or sqrt(x[i]) for normal x > 0 (which = 2) as every kernel
+ * evaluates the radicand of Eq. 4.  Lets tests check them in isolation.       */
 int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream);
 
 #ifdef __cplusplus

@@ -930,11 +930,11 @@ int fe_fp64_peak_probe(int32_t blocks, int32_t iters, float* ms, double* dfma_co
   return FE_OK;
 }
 
-// Diagnostic entry used by the GPU tests: y[i] = exp_nonpos(x[i]) (which = 0) or log_1p_w(x[i]) (which = 1).
+// Diagnostic entry used by the GPU tests: y[i] = exp_nonpos(x[i]) (which = 0), log_1p_w(x[i]) (which = 1), sqrt_pos(x[i]) (2).
 // x_dev, y_dev: DEVICE arrays of n doubles.  Not part of the method; exported so the device math can be
 // checked in isolation against numpy.
 int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, double* y_dev, void* cuda_stream) {
-  if (!h || !x_dev || !y_dev || n < 1 || (which != 0 && which != 1)) { snprintf(g_errbuf, sizeof g_errbuf, "bad argument"); return FE_EINVAL; }
+  if (!h || !x_dev || !y_dev || n < 1 || which < 0 || which > 2) { snprintf(g_errbuf, sizeof g_errbuf, "bad argument"); return FE_EINVAL; }
   fe_math_probe_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(which, n, x_dev, y_dev, h->d_tabs);
   FE_CUDA(cudaGetLastError());
   h->launches++;

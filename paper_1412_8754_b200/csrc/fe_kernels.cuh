@@ -52,19 +52,20 @@ struct KsumParams {
   double* partial;                     // [ksplit][nq*nh*nd]
 };
 
-// Branch-free sqrt for normal x > 0 (callers add 1e-300 to the radicand so x = 0 cannot occur): rsqrt seed (MUFU,
-// ~2^-22) and two coupled Newton steps (error 2^-43, then 2^-85 + rounding): <= 1.5 ulp, no slow path, so
-// independent chains interleave.  7 FP64 instructions.
+// Branch-free sqrt for normal x > 0 (callers add 1e-300 to the radicand so x = 0 cannot occur): rsqrt seed y (MUFU,
+// ~2^-22), one coupled Newton step g1 = g0 + g0 (1/2 - g0 h0) with g0 = x y, h0 = y/2 (error 1.5 e^2 ~ 2^-43), then the
+// exact-residual correction g2 = g1 + h0 (x - g1^2): the residual is formed exactly by the FMA, and the 2^-22 error of
+// h0 only scales a 2^-43 correction, so g2 is sqrt(x) to 2^-65 before its single final rounding (<= 0.5 ulp + 2^-12 ulp).
+// No slow path, so independent chains interleave.  5 FP64 instructions: y/2 is an integer subtraction on the exponent.
 __device__ __forceinline__ double sqrt_pos(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = __hiloint2double(__double2hiint(y) - 0x00100000, __double2loint(y));   // y / 2 (y is normal, far from underflow)
   double g = x * y;            // ~ sqrt(x)
-  double h = 0.5 * y;          // ~ 1 / (2 sqrt(x))
-  double r = fma(-g, h, 0.5);
+  const double r = fma(-g, h, 0.5);
   g = fma(g, r, g);
-  h = fma(h, r, h);
-  r = fma(-g, h, 0.5);
-  return fma(g, r, g);
+  const double d = fma(-g, g, x);
+  return fma(d, h, g);
 }
 
 // 1/x and 1/sqrt(x) for normal x without the slow-path branches of the IEEE division / sqrt: MUFU seed (~2^-22) and
@@ -760,7 +761,7 @@ __global__ void fe_math_probe_kernel(int which, int n, const double* __restrict_
   __syncthreads();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  y[i] = which == 0 ? exp_nonpos(x[i], tabs) : log_1p_w(x[i], tabs);
+  y[i] = which == 0 ? exp_nonpos(x[i], tabs) : (which == 1 ? log_1p_w(x[i], tabs) : sqrt_pos(x[i]));
 }
 #endif  // FE_PLAIN_KERNELS
 

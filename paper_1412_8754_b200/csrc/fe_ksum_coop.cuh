@@ -60,9 +60,14 @@ struct __align__(16) CoopHdr {         // one per (k, band) slot
   int flags;                           // bit 0 skip, bit 1 robust, bits 8.. = drift step
 };
 constexpr int kCoopSkip = 1, kCoopRobust = 2;
-// A slot is "A-dominated" when over the whole block tile 2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^kDomGap:
-// then Z_ij = A_j and 2cosh(R_j/T) = e^{R_j/T} to beyond fp64, so T ln Z_ij = R_j for every pair (neglected: < T 2^-56).
-constexpr int kDomGap = 58;
+// A slot is "A-dominated" when over the whole block tile the binary exponent of 2cosh(R_j/T) exceeds that of 2cosh(|d_i|/T)
+// by kDomGap or more (mantissas are in [0.997, 2.51), so A_j / B_i > 2^(kDomGap - 1.4)): then T ln Z_ij is replaced by R_j
+// for every pair.  What is neglected per term is T ln(1 + B_i/A_j) + T ln(1 + e^{-2R_j/T}) < T 2^-(kDomGap - 1.4) (1 + tiny),
+// and a slot can only be dominated if e^{R_j/T} > 2^(kDomGap - 1.4), i.e. T < R_j / ((kDomGap - 1.4) ln 2): the neglected part
+// is below R_j 2^-48.6 / (48.6 ln 2) = 6.9e-17 R_j < 2^-53 R_j, less than half an ulp of the term it belongs to, in the
+// worst case of a pair sitting exactly at the threshold (pairs are spread over thousands of T beyond it, so the sum of what
+// is neglected is orders of magnitude smaller still).  Same bound for the B-dominated slots (T ln Z_ij = |d_i|).
+constexpr int kDomGap = 50;
 
 template <int TH, int TD, int LH, int NW, int KB, int NB>
 struct CoopGeom {

@@ -615,6 +615,13 @@ def test_device_math(fe):
         l = F.debug_math(1, torch.from_numpy(wv).cuda()).cpu().numpy()
         refl = np.log1p(wv)
         assert np.max(np.abs(l - refl)) < 2.5e-16                           # absolute error bound
+        # sqrt of the Eq. 4 radicand (rsqrt seed + one Newton step + exact-residual correction): correctly rounded up to
+        # 2^-12 ulp, over the whole range the radicands can take (1e-300 floor ... band width squared)
+        xs = np.concatenate([rng.uniform(0, 100, 400000), 10 ** rng.uniform(-300, 8, 400000), [1e-300, 1.0, 4.0, 2.0, 1e-8]])
+        r = F.debug_math(2, torch.from_numpy(xs).cuda()).cpu().numpy()
+        refs = np.sqrt(xs)
+        assert np.max(np.abs(r - refs) / np.spacing(refs)) <= 1.0
+        assert np.mean(r == refs) > 0.999
 
 
 # --------------------------------------------------------------------------------------------------
