@@ -453,7 +453,7 @@ def main():
     ap.add_argument("--steps", type=int, default=6)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="coop_eo", choices=["coop_eo", "coop", "factored", "direct", "windowed", "sp", "spfm", "verified_sp", "verified_spfm", "verified_mixed"],
+    ap.add_argument("--mode", default="coop_eo", choices=["coop_eo", "coop", "factored", "direct", "windowed", "sp", "spfm", "verified_sp", "verified_spfm"],
                     help="coop_eo = library default (early-out); coop = dense variant (every pair multiplied out)")
     ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
                     help="N > 1 GPUs: strong = the config's own q list split round-robin over the ranks; weak = every rank scans the whole q list")
@@ -503,7 +503,7 @@ def main():
     nq_rank = len(q_all)
     nq_step = min(args.q_per_step or nq_rank, max(nq_rank, 1))
     temps = list(w.T)
-    sp_mode = args.mode in ("sp", "spfm", "verified_sp", "verified_spfm", "verified_mixed")
+    sp_mode = args.mode in ("sp", "spfm", "verified_sp", "verified_spfm")   # the paper's SP / SPFM builds
     mode = {"coop": fe.EVAL_COOP, "factored": fe.EVAL_FACTORED, "direct": fe.EVAL_DIRECT,
             "windowed": fe.EVAL_WINDOWED}.get(args.mode, fe.EVAL_COOP_EO)
 
@@ -529,9 +529,10 @@ def main():
         if args.mode in ("sp", "spfm"):
             F.omega_grid_sp(q_of(step), w.h, w.delta, fast_math=args.mode == "spfm", out=omega, stream=stream)
         elif sp_mode:
-            r = F.scan_verified(q_of(step), w.h, w.delta, screen={"verified_sp": "sp", "verified_spfm": "spfm",
-                                                                   "verified_mixed": "mixed"}[args.mode], stream=stream)
-            verified.append(r[3])
+            r = F.scan_verified(q_of(step), w.h, w.delta, screen={"verified_sp": "sp", "verified_spfm": "spfm"}[args.mode],
+                                stream=stream)
+            verified.append({"delta_values_verified_in_fp64": r[3], "of": w.nd, "columns_whose_minimum_moved": r[4],
+                             "columns": nq_step * w.nh})
             return r[:3]
         else:
             F.omega_grid(q_of(step), w.h, w.delta, out=omega, stream=stream)
@@ -556,6 +557,7 @@ def main():
     sampler.start()
     launches0 = F.launch_count()
     step_ms, ksum_ms, step_T, band_evals = [], [], [], 0.0
+    slot_kinds = {}                                     # per temperature: what the timed launches were made of (in-run counters)
     res = None
     barrier()
     t_wall0 = time.perf_counter()
@@ -572,6 +574,10 @@ def main():
             ms, be = F.last_ksum()
             ksum_ms.append(ms)
             band_evals = be
+            if args.mode in ("coop", "coop_eo"):
+                c = F.slot_counts()                     # device -> host read of four counters, outside the events
+                tot = sum(c.values()) - c["padding"]
+                slot_kinds[f"T={step_T[-1]:g}"] = {k: v / tot for k, v in c.items()}
     barrier()
     t_wall = time.perf_counter() - t_wall0
     launches = F.launch_count() - launches0
@@ -673,6 +679,10 @@ def main():
     roofline = roofline_base(f"k-sum kernel ({args.mode}, tile {info['th']}x{info['td']}, grid {info['grid']} x {info['block']})", dfma_rate)
     roofline.update({"avg_launch_ms": k_ms, "median_launch_ms": statistics.median(ksum_ms), "band_evals_per_launch": band_evals,
                      "kernel_share_of_step": sum(ksum_ms) / total_ms})
+    if slot_kinds:
+        roofline["slot_kinds"] = {"what": "fractions of the (k, band, block tile) slots of a timed launch, counted by the kernel in this run: "
+                                          "dense slots (and padding, relative to the same total) run through the pair products, "
+                                          "dominated slots are summed without exponentials", **slot_kinds}
     if sp_mode:
         roofline["note"] = ("lower-precision builds (SURVEY 8f-2): see profiles/; avg_launch_ms is the last k-sum launch of a step "
                             "(verified_*: the fp64 pass on the candidate list); fp64-verified Delta values per step: " + str(verified[-4:]))

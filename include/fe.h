@@ -151,18 +151,23 @@ int fe_omega_grid_sp(fe_handle* h,
 
 /* Low-precision screening + selective double-precision verification ("run larger parameter scans at
  * lower precision and then selectively verify with double precision calculations"):
- *   1. fe_omega_grid_sp over the whole grid;  2. every Delta index that comes within margin_rel * |min| of the minimum
- *   of ANY (q, h) column is a candidate;  3. fe_omega_grid (fp64, the handle's evaluation mode) on the candidate Delta
- *   list only;  4. fe_argmin on that, indices mapped back to the full list.
- * The minima equal those of a full fp64 scan whenever the single-precision error is below margin_rel / 2 (1e-5 is
- * ample: measured error ~1e-7).  All list pointers HOST; idx_dev / delta_star_dev / omega_star_dev DEVICE, nq*nh each,
- * any may be NULL; *n_verified_host (HOST, may be NULL) receives the number of Delta values evaluated in fp64.
- * Synchronises the stream once between steps 2 and 3 (the candidate list is built on the host).            */
+ *   1. fe_omega_grid_sp over the whole grid;  2. every Delta index that comes within margin_rel * M of the minimum of ANY
+ *   (q, h) column is a candidate, M = max(|column minimum|, N^2 (#bands in band_mask) (band half-width + |mu|)): the
+ *   single-precision error scales with the magnitude of the summed terms, not with |Omega_min|, which may be near zero;
+ *   3. fe_omega_grid (fp64, the handle's evaluation mode) on the candidate Delta list only;  4. fe_argmin on that, indices
+ *   mapped back to the full list.
+ * Guarantee: the minima equal those of a full fp64 scan whenever the single-precision Omega is within margin_rel * M / 2 of
+ * the fp64 Omega on every grid point (measured error ~1e-7 M: the default 1e-5 is ample).  All list pointers HOST;
+ * idx_dev / delta_star_dev / omega_star_dev DEVICE, nq*nh each, any may be NULL; HOST outputs, either may be NULL:
+ * *n_verified_host = number of Delta values evaluated in fp64; *n_changed_host = number of (q, h) columns whose minimum
+ * index the verification moved away from the single-precision argmin (-1 if idx_dev is NULL) -- the quantity PAPER.md:198
+ * asks to watch ("we advise careful experimentation").  Synchronises the stream between steps 2 and 3 (the candidate list
+ * is built on the host) and before returning.            */
 int fe_scan_verified(fe_handle* h,
                      const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                      const double* delta, int32_t nd, int32_t fast_math, double margin_rel,
                      int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev,
-                     int32_t* n_verified_host, void* cuda_stream);
+                     int32_t* n_verified_host, int32_t* n_changed_host, void* cuda_stream);
 
 /* Host-buffer end-to-end path: copies the lists to the device, runs fe_omega_grid and fe_argmin,
  * copies results back and SYNCHRONISES the stream.  All pointers are HOST memory (pinned or pageable).
@@ -179,6 +184,13 @@ int fe_scan_host(fe_handle* h,
  * the duration of the most recent K1 launch (ms) and the number of (k, band, q, h, Delta) terms it evaluated. */
 int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
+
+/* What the most recent TIMED cooperative k-sum launch (FE_EVAL_COOP / FE_EVAL_COOP_EO with fe_enable_timing on) was made
+ * of: counts4 = {dense, A-dominated, B-dominated, padding} (k, band) slots, each counted once per block tile it was
+ * classified for (a slot of a 64 x 128 block tile stands for 8192 (h, Delta) pairs).  Dense and padding slots run through
+ * the pair products, dominated slots are summed without exponentials (FE_EVAL_COOP_EO; FE_EVAL_COOP has none).  HOST
+ * doubles; call after synchronising the stream (the call copies four counters from the device).  FE_EINVAL if there is none. */
+int fe_get_slot_counts(fe_handle* h, double* counts4);
 
 /* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode actually
  * used, rows per k-chunk}; for FE_EVAL_COOP / FE_EVAL_COOP_EO: {WH, WD, ksplit, grid blocks, mode, k-points per chunk};

@@ -97,6 +97,8 @@ struct fe_handle {
   bool timing_valid = false;
   double last_band_evals = 0;
   int32_t last_info[6] = {0, 0, 0, 0, 0, 0};   // th, td, ksplit, grid, mode, rows_per_chunk
+  unsigned long long* d_kinds = nullptr;       // 4 slot-kind counters of the most recent timed K1c launch
+  bool kinds_valid = false;
   int64_t launches = 0;
 };
 
@@ -526,6 +528,14 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     h->last_info[5] = (int32_t)(CP.kc < 2147483647ULL ? CP.kc : 2147483647ULL);          // k-points per chunk
     CP.coltab = h->d_coltab; CP.rowtab = h->d_rowtab; CP.h = d_h; CP.d2 = d_d2; CP.tabs = h->d_tabs;
     CP.partial = h->d_partial; CP.etab = h->d_etab;
+    CP.kind_counts = nullptr;
+    h->kinds_valid = false;
+    if (h->timing) {
+      if (!h->d_kinds) FE_CUDA(cudaMalloc((void**)&h->d_kinds, 4 * sizeof(unsigned long long)));
+      FE_CUDA(cudaMemsetAsync(h->d_kinds, 0, 4 * sizeof(unsigned long long), st));
+      CP.kind_counts = h->d_kinds;
+      h->kinds_valid = true;
+    }
   }
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
   if (sp) {
@@ -790,8 +800,9 @@ int fe_omega_grid_sp(fe_handle* h, const double* q_xy, int32_t nq, const double*
 int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
                      const double* delta, int32_t nd, int32_t fast_math, double margin_rel,
                      int32_t* idx_dev, double* delta_star_dev, double* omega_star_dev,
-                     int32_t* n_verified_host, void* cuda_stream) {
+                     int32_t* n_verified_host, int32_t* n_changed_host, void* cuda_stream) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  if (n_changed_host) *n_changed_host = -1;
   if (fast_math != 0 && fast_math != 1) { snprintf(g_errbuf, sizeof g_errbuf, "fast_math must be 0 or 1"); return FE_EINVAL; }
   if (!(margin_rel >= 0.0) || !isfinite(margin_rel)) { snprintf(g_errbuf, sizeof g_errbuf, "margin_rel must be finite and >= 0"); return FE_EINVAL; }
   int rc = check_lists(q_xy, nq, h_list, nh, delta, nd);
@@ -800,7 +811,11 @@ int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double*
   const size_t nout = (size_t)nq * nh * nd;
   const int ncol = nq * nh;
   if ((rc = ensure(h->d_omega, h->omega_cap, nout))) return rc;
-  if ((rc = ensure(h->d_flags, h->flags_cap, (size_t)(nd > ncol ? nd : ncol)))) return rc;
+  // flags: [0, max(nd, ncol)) candidate flags then the index map; behind it ncol low-precision minima and one counter
+  const size_t nflag = (size_t)(nd > ncol ? nd : ncol);
+  if ((rc = ensure(h->d_flags, h->flags_cap, nflag + (size_t)ncol + 1))) return rc;
+  int32_t* const d_idx_lo = h->d_flags + nflag;
+  int32_t* const d_changed = d_idx_lo + ncol;
   if ((size_t)nd > h->hflags_cap) {
     if (h->h_flags) cudaFreeHost(h->h_flags);
     h->h_flags = nullptr; h->hflags_cap = 0;
@@ -810,6 +825,10 @@ int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double*
   }
   // 1. screening pass in single precision
   if ((rc = omega_grid_impl(h, q_xy, nq, h_list, nh, delta, nd, h->d_omega, st, 1 + fast_math))) return rc;
+  if (n_changed_host && idx_dev) {           // the screening pass's own minima, to report how many the verification moves
+    if ((rc = argmin_impl(h, h->d_omega, delta, ncol, nd, d_idx_lo, nullptr, nullptr, st))) return rc;
+    FE_CUDA(cudaMemsetAsync(d_changed, 0, sizeof(int32_t), st));
+  }
   // 2. candidates
   FE_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * (size_t)nd, st));
   // the low-precision error scales with the magnitude of the summed terms (~ N^2 (band half-width + |mu|) per band),
@@ -840,6 +859,12 @@ int fe_scan_verified(fe_handle* h, const double* q_xy, int32_t nq, const double*
     fe_map_index_kernel<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, h->d_flags, idx_dev);
     FE_CUDA(cudaGetLastError());
     h->launches++;
+    if (n_changed_host) {
+      fe_count_changed_kernel<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, d_idx_lo, idx_dev, d_changed);
+      FE_CUDA(cudaGetLastError());
+      h->launches++;
+      FE_CUDA(cudaMemcpyAsync(n_changed_host, d_changed, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    }
     FE_CUDA(cudaStreamSynchronize(st));        // h_flags (pinned map) may be reused by the next call
   }
   return FE_OK;
@@ -896,6 +921,15 @@ int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
   return FE_OK;
 }
 
+int fe_get_slot_counts(fe_handle* h, double* counts4) {
+  if (!h || !counts4) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+  if (!h->kinds_valid || !h->d_kinds) { snprintf(g_errbuf, sizeof g_errbuf, "no timed cooperative k-sum launch recorded"); return FE_EINVAL; }
+  unsigned long long c[4];
+  FE_CUDA(cudaMemcpy(c, h->d_kinds, sizeof c, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < 4; ++i) counts4[i] = (double)c[i];
+  return FE_OK;
+}
+
 int fe_get_last_launch_info(fe_handle* h, int32_t* info6) {
   if (!h || !info6) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
   for (int i = 0; i < 6; ++i) info6[i] = h->last_info[i];
@@ -944,6 +978,7 @@ int fe_debug_math(fe_handle* h, int32_t which, int32_t n, const double* x_dev, d
 void fe_destroy(fe_handle* h) {
   if (!h) return;
   cudaFree(h->d_tabs); cudaFree(h->d_coltab); cudaFree(h->d_rowtab); cudaFree(h->d_partial);
+  cudaFree(h->d_kinds);
   cudaFree(h->d_spart); cudaFree(h->d_etab); cudaFree(h->d_omega); cudaFree(h->d_omega2); cudaFree(h->d_flags);
   if (h->h_flags) cudaFreeHost(h->h_flags); cudaFree(h->d_res);
   for (auto& s : h->slots) {

@@ -731,6 +731,15 @@ __global__ void fe_map_index_kernel(int ncol, const int32_t* __restrict__ map, i
   if (c < ncol) idx[c] = map[idx[c]];
 }
 
+// K7: how many columns changed their minimum when the low-precision argmin was verified in fp64 (exact integer count)
+__global__ void fe_count_changed_kernel(int ncol, const int32_t* __restrict__ idx_lo, const int32_t* __restrict__ idx_hi,
+                                        int32_t* __restrict__ count) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool diff = c < ncol && idx_lo[c] != idx_hi[c];
+  const unsigned m = __ballot_sync(0xffffffffu, diff);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, __popc(m));
+}
+
 // ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 16 independent DFMA chains per thread, register-resident.
 // ---------------------------------------------------------------------------------------------------

@@ -52,6 +52,8 @@ struct CoopParams {
   const MathTabs* tabs;
   const double* etab;                  // NB == 3 only: [1 + nq][3][N*N] band tables, y = 0: E(k), 1 + iq: E(k - q)
   double* partial;                     // [ksplit][nq*nh*nd]
+  unsigned long long* kind_counts;     // NULL, or 4 device counters {dense, A-dominated, B-dominated, padding} slots, summed
+                                       // over all blocks of the launch (fe_enable_timing; block-tile slots of WH x WD pairs)
 };
 
 struct __align__(16) CoopHdr {         // one per (k, band) slot
@@ -262,6 +264,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       hdr_s[ndense + tid] = z;
     }
     const bool rob = __syncthreads_or(any_robust) != 0;
+    if (P.kind_counts != nullptr && tid == 0) {              // diagnostics only (fe_enable_timing): what the launch was made of
+      if (ndense) atomicAdd(P.kind_counts + 0, (unsigned long long)ndense);
+      if (ndom) atomicAdd(P.kind_counts + 1, (unsigned long long)ndom);
+      if (ndomB) atomicAdd(P.kind_counts + 2, (unsigned long long)ndomB);
+      if (nsub * SLOTS - ndense) atomicAdd(P.kind_counts + 3, (unsigned long long)(nsub * SLOTS - ndense));
+    }
     // A-dominated slots: T ln Z_ij = R_j for the whole tile (kDomGap); this thread owns Delta_j, j = tid + r NT
     if (ndom > 0) {
       const CoopHdr* const dm = hdr_s + (G::HTOT - ndom);

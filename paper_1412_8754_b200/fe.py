@@ -19,7 +19,7 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 # include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
-               "fe_get_launch_count", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
+               "fe_get_launch_count", "fe_get_slot_counts", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
@@ -67,12 +67,13 @@ def lib():
     L.fe_pair_susceptibility.argtypes = [vp, dp, C.c_int32, C.c_double, vp, vp]
     L.fe_omega_grid_sp.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, C.c_int32, vp, vp]
     L.fe_scan_verified.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, C.c_int32, C.c_double, vp, vp, vp,
-                                   C.POINTER(C.c_int32), vp]
+                                   C.POINTER(C.c_int32), C.POINTER(C.c_int32), vp]
     L.fe_scan_host.argtypes = [vp, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, vp, vp, vp, vp, vp]
     L.fe_enable_timing.argtypes = [vp, C.c_int32]
     L.fe_get_timing.argtypes = [vp, C.POINTER(C.c_float), dp]
     L.fe_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.fe_get_last_launch_info.argtypes = [vp, ip]
+    L.fe_get_slot_counts.argtypes = [vp, dp]
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
     L.fe_set_debug_flags.argtypes = [vp, C.c_int32]
@@ -214,6 +215,12 @@ class FreeEnergy:
         _check(lib().fe_get_last_launch_info(self._h, a))
         return dict(th=a[0], td=a[1], ksplit=a[2], grid=a[3], mode=a[4], rows_per_chunk=a[5])
 
+    def slot_counts(self):
+        """{dense, a_dominated, b_dominated, padding} slot counts of the most recent timed cooperative k-sum launch."""
+        a = (C.c_double * 4)()
+        _check(lib().fe_get_slot_counts(self._h, a))
+        return dict(dense=a[0], a_dominated=a[1], b_dominated=a[2], padding=a[3])
+
     def launch_count(self):
         n = C.c_int64()
         _check(lib().fe_get_launch_count(self._h, C.byref(n)))
@@ -286,7 +293,8 @@ class FreeEnergy:
         return out
 
     def scan_verified(self, q, h, delta, fast_math=False, margin_rel=1e-5, stream=None, screen=None):
-        """Low-precision screening + fp64 verification of the candidates: (idx, delta*, omega*, n_verified).
+        """Low-precision screening + fp64 verification of the candidates: (idx, delta*, omega*, n_verified, n_changed);
+        n_changed = columns whose minimum the fp64 verification moved away from the single-precision argmin.
         screen: "sp" | "spfm" (the paper's single-precision builds) -- overrides fast_math when given."""
         import torch
         if screen is not None:
@@ -296,11 +304,12 @@ class FreeEnergy:
         idx = torch.empty(shp, dtype=torch.int32, device="cuda")
         ds = torch.empty(shp, dtype=torch.float64, device="cuda")
         os_ = torch.empty(shp, dtype=torch.float64, device="cuda")
-        nv = C.c_int32(0)
+        nv, nc = C.c_int32(0), C.c_int32(0)
         _check(lib().fe_scan_verified(self._h, _dptr(q), q.shape[0], _dptr(h), h.shape[0], _dptr(d), d.shape[0],
                                       int(bool(fast_math)), float(margin_rel), C.c_void_p(idx.data_ptr()),
-                                      C.c_void_p(ds.data_ptr()), C.c_void_p(os_.data_ptr()), C.byref(nv), _stream(stream)))
-        return idx, ds, os_, nv.value
+                                      C.c_void_p(ds.data_ptr()), C.c_void_p(os_.data_ptr()), C.byref(nv), C.byref(nc),
+                                      _stream(stream)))
+        return idx, ds, os_, nv.value, nc.value
 
     def scan_host(self, q, h, delta, want_omega=True, out=None, stream=None):
         """Host-buffer end-to-end path (fe_scan_host): numpy in, numpy out, synchronous.

@@ -363,11 +363,14 @@ def test_scan_verified_equals_full_fp64_scan(fe, oracle, fast):
                  (W.ragged(seed=7, N=45, nq=3, nh=5, nd=37), 0.004), (W.config(2), 0.001)):
         ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
         with fe.FreeEnergy(w.params, w.N, T) as F:
-            idx, ds, os_, nver = F.scan_verified(w.q, w.h, w.delta, fast_math=fast)
+            idx, ds, os_, nver, nchanged = F.scan_verified(w.q, w.h, w.delta, fast_math=fast)
             om = F.omega_grid(w.q, w.h, w.delta)
             fidx, fds, fos = F.argmin(om, w.delta)
+            sidx = F.argmin(F.omega_grid_sp(w.q, w.h, w.delta, fast_math=fast), w.delta)[0]
             torch.cuda.synchronize()
         assert 1 <= nver <= w.nd
+        # the library's report of where single precision gets the minimum wrong is an exact count
+        assert nchanged == int((sidx != idx).sum().item())
         check_argmin(ref, w.delta, idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy())      # vs the fp64 oracle
         # and against the library's own full fp64 scan: same minima wherever they are resolved
         same = idx.cpu().numpy() == fidx.cpu().numpy()
@@ -377,6 +380,19 @@ def test_scan_verified_equals_full_fp64_scan(fe, oracle, fast):
     w = W.interior_minimum(N=64, U=5.0, T=0.001, nq=2, nh=4, nd=200)
     with fe.FreeEnergy(w.params, w.N, 0.001) as F:
         nver = F.scan_verified(w.q, w.h[:2], w.delta, fast_math=fast, margin_rel=1e-5)[3]
+        # a column minimum near zero (one nearly empty band: the k-sum cancels against the condensation term): the margin is
+        # relative to the magnitude of the summed terms, so the verified minima still equal the full fp64 scan's
+        p0 = dict(W.model_params(U=5.0), band_mask=1, cond_mult=1.0, mu=1.15)       # just below the bottom of band E_+ (1.2)
+        w0 = W.Workload("near_zero_min", p0, 48, (0.002,), w.q[:2], np.linspace(0.0, 0.2, 6), np.linspace(0.0, 0.5, 120))
+        with fe.FreeEnergy(w0.params, w0.N, 0.002) as F0:
+            vi, _, vo, nv0, _ = F0.scan_verified(w0.q, w0.h, w0.delta, fast_math=fast)
+            fo = F0.omega_grid(w0.q, w0.h, w0.delta)
+            fi, _, fos0 = F0.argmin(fo, w0.delta)
+            torch.cuda.synchronize()
+        fmin = fos0.cpu().numpy()
+        assert np.all(np.abs(fmin) < 1e-3 * 9.0 * 48 * 48)             # |Omega_min| is < 1e-3 of the summed magnitude
+        assert torch.equal(vi, fi) and nv0 >= 1
+        assert np.all(np.abs(vo.cpu().numpy() - fmin) <= 1e-9 * np.abs(fmin))   # (cancelling sum: cond ~ 1e3, two summation trees)
         with pytest.raises(fe.FeError):
             F.scan_verified(w.q, w.h, w.delta, margin_rel=-1.0)
     assert nver < w.nd // 2, nver
