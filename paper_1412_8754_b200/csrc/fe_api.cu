@@ -451,8 +451,10 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     if (h->target_blocks > 0) {
       ks = (h->target_blocks + ctiles - 1) / ctiles;
     } else {
-      // >= 8 waves; among the next candidates take the split whose last wave is fullest
-      const long long ks0 = (8 * wave + ctiles - 1) / ctiles;
+      // >= 24 waves (the dense share of a k-chunk varies with where it lies in the zone, so block durations differ: many
+      // short blocks keep the last waves full; measured on the config-4 step: 8 waves 71.0 / 102.4 ms, 24 waves 69.3 / 99.8 ms
+      // for T = 0.001 / 0.01); among the next candidates take the split whose last wave is fullest
+      const long long ks0 = (24 * wave + ctiles - 1) / ctiles;
       ks = ks0; double best_eff = 0;
       for (long long c = ks0; c <= 2 * ks0 + 1; ++c) {
         const long long g = ctiles * c, waves = (g + wave - 1) / wave;

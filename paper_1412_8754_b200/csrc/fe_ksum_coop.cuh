@@ -82,8 +82,9 @@ struct CoopGeom {
   static constexpr int W = WD + LH * (TH + PADB);            // doubles per slot row
   static constexpr int SLOTS = KB * NB;        // slots per sub-batch
   static constexpr int BUF_DOUBLES = SLOTS * W + SLOTS;      // values + one int2 {eref, flags} per slot
-  static constexpr int HTOT = NT * NB + SLOTS;  // header array: dense slots compacted at the front (padded to whole
-                                               // sub-batches), A-dominated slots at the back
+  static constexpr int DPAD = 16;              // room behind the A-dominated list: its neutral padding (< 8) + one prefetch round (8)
+  static constexpr int HTOT = NT * NB + SLOTS + DPAD;   // header array: dense slots compacted at the front (padded to whole
+                                               // sub-batches), B- then A-dominated slots at the back
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
       sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT) + sizeof(int) * 2 * (NW + 2);
@@ -250,8 +251,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     const int nsub = (ndense + SLOTS - 1) / SLOTS;
     const int off = base + incl - cnt;                       // exclusive prefix of the three counts
     int pd = off & 0x3ff;                                    // first dense position of this thread
-    int pm = G::HTOT - ndom + ((off >> 10) & 0x3ff);         // first A-dominated position (back of the array)
-    int pb = G::HTOT - ndom - ndomB + (off >> 20);           // first B-dominated position (just before them)
+    constexpr int DEND = G::HTOT - G::DPAD;                  // end of the A-dominated list
+    int pm = DEND - ndom + ((off >> 10) & 0x3ff);            // first A-dominated position (back of the array)
+    int pb = DEND - ndom - ndomB + (off >> 20);              // first B-dominated position (just before them)
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
       if (kind[e] == 1) hdr_s[pd++] = hd[e];
@@ -263,6 +265,11 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       z.s2 = 1.0; z.g2 = 0.0; z.d0 = 0.0; z.eref = 0; z.flags = kCoopSkip;
       hdr_s[ndense + tid] = z;
     }
+    if (tid < ((8 - (ndom & 7)) & 7)) {                      // the A-dominated list is summed 8 entries at a time: pad it with
+      CoopHdr z;                                             // entries that add sqrt(1e-300) = 1e-150 to a sum of O(1) terms
+      z.s2 = 1e-300; z.g2 = 0.0; z.d0 = 0.0; z.eref = 0; z.flags = kCoopSkip;
+      hdr_s[DEND + tid] = z;
+    }
     const bool rob = __syncthreads_or(any_robust) != 0;
     if (P.kind_counts != nullptr && tid == 0) {              // diagnostics only (fe_enable_timing): what the launch was made of
       if (ndense) atomicAdd(P.kind_counts + 0, (unsigned long long)ndense);
@@ -272,30 +279,29 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     }
     // A-dominated slots: T ln Z_ij = R_j for the whole tile (kDomGap); this thread owns Delta_j, j = tid + r NT
     if (ndom > 0) {
-      const CoopHdr* const dm = hdr_s + (G::HTOT - ndom);
+      // entries 0 .. ndom - 1, then the neutral padding up to a multiple of 8; the fetch runs one round ahead (the last
+      // round reads 8 entries past the padding: still inside hdr_s, never used)
+      const double2* const dm = reinterpret_cast<const double2*>(&hdr_s[DEND - ndom].s2);   // entry i at dm[2 i]: {s2, g2}
 #pragma unroll 1
       for (int r = 0; r < WD / NT; ++r) {
         const double d2 = d2_s[tid + r * NT];
         constexpr int UD = 8;                                // independent sqrt chains, fixed order
         double acc[UD];
-        double2 g[UD];                                       // headers are fetched one round ahead of their use
-        auto ld = [&](int i) { return *reinterpret_cast<const double2*>(&dm[min(i, ndom - 1)].s2); };
+        double2 g[UD];
+        const double2* p = dm;
 #pragma unroll
-        for (int u = 0; u < UD; ++u) { acc[u] = 0.0; g[u] = ld(u); }
-        int i = 0;
+        for (int u = 0; u < UD; ++u) { acc[u] = 0.0; g[u] = p[2 * u]; }
 #pragma unroll 1
-        for (; i + UD <= ndom; i += UD) {
+        for (int i = 0; i < ndom; i += UD) {
           double2 n[UD];
+          p += 2 * UD;
 #pragma unroll
-          for (int u = 0; u < UD; ++u) n[u] = ld(i + UD + u);
+          for (int u = 0; u < UD; ++u) n[u] = p[2 * u];
 #pragma unroll
           for (int u = 0; u < UD; ++u) acc[u] += sqrt_pos(fma(d2, g[u].y, g[u].x));       // R_j, Eq. 4 radicand   (S5)
 #pragma unroll
           for (int u = 0; u < UD; ++u) g[u] = n[u];
         }
-#pragma unroll
-        for (int u = 0; u < UD - 1; ++u)                     // tail: g[u] holds entry i + u (clamped loads)
-          if (i + u < ndom) acc[u] += sqrt_pos(fma(d2, g[u].y, g[u].x));
         const double a0 = acc[0] + acc[4], a1 = acc[1] + acc[5], a2 = acc[2] + acc[6], a3 = acc[3] + acc[7];
         accR_s[tid + r * NT] += (a0 + a1) + (a2 + a3);
       }
@@ -303,7 +309,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     // B-dominated slots (2cosh(|d_i|/T) exceeds 2cosh(R_j/T) by 2^kDomGap over the whole tile): T ln Z_ij = |d0 - h_i|
     // for every Delta_j.  Thread (half, ib) = (tid / WH, tid % WH) sums every (NT / WH)-th entry for its h_i.
     if (ndomB > 0) {
-      const CoopHdr* const db = hdr_s + (G::HTOT - ndom - ndomB);
+      const CoopHdr* const db = hdr_s + (DEND - ndom - ndomB);
       const double hv = h_s[tid % WH];
       double a0 = 0.0, a1 = 0.0;
       int i = tid / WH;
