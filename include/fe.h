@@ -137,7 +137,10 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
  *   q_xy    : HOST, nq pairs (qx, qy), any real vectors (copied before return).
  *   chi_dev : DEVICE, nq * nb * nb doubles, index (iq*nb + e)*nb + f, nb = number of bands (band_mask is ignored).
  * Asynchronous on cuda_stream; deterministic.  With fe_enable_timing the k-sum kernel of this call is the one
- * fe_get_timing reports (its second value is then the number of (k, q, e, f) pair terms).               */
+ * fe_get_timing reports (its second value is then the number of (k, q, e, f) pair terms).  Three-band model: q-values on
+ * the k-grid read the unshifted band table at a shifted index; q-values off the grid need a table each (3 N^2 doubles),
+ * so the list is worked through in consecutive slices whose tables fit ~2 GB of scratch (fe_get_timing then reports the
+ * last slice).               */
 int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream);
 
 /* The paper's single-precision builds: Omega on the full grid with every per-term

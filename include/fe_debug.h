@@ -39,6 +39,10 @@ int fe_coop_shape_info(int32_t shape, int32_t* info6);
  * sums; only the code path changes (lets tests cover each path).                                            */
 int fe_set_debug_flags(fe_handle* h, int32_t flags);
 
+/* fe_pair_susceptibility, three-band model: bytes of per-q band tables one slice of the q list may hold (default 2e9;
+ * a slice always holds at least one off-grid q).  Lets tests force the slicing on small grids.  Results do not depend on it. */
+int fe_set_chi_table_budget(fe_handle* h, double bytes);
+
 /* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
  * y[i] = exp(x[i]) for x <= 0 (which = 0), ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the direct k-sum
  * kernel evaluates the thermal term of Eq. 5, or sqrt(x[i]) for normal x > 0 (which = 2) as every kernel

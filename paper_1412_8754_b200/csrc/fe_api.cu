@@ -64,6 +64,7 @@ struct fe_handle {
   int32_t target_blocks = 0;   // 0 = auto
   int32_t debug_flags = 0;
   int32_t coop_shape = 0;      // 0 = auto, else 1 + index into kCoopShapes
+  double chi_table_budget = 2.0e9;   // bytes of band tables one slice of fe_pair_susceptibility may hold (three-band model)
   int device = 0;
   int sm_count = 148;
   int nb = 1;
@@ -667,6 +668,12 @@ int fe_coop_shape_info(int32_t shape, int32_t* info6) {
   return FE_OK;
 }
 
+int fe_set_chi_table_budget(fe_handle* h, double bytes) {
+  if (!h || !(bytes >= 0.0) || !isfinite(bytes)) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL or bytes is not finite and >= 0"); return FE_EINVAL; }
+  h->chi_table_budget = bytes;
+  return FE_OK;
+}
+
 int fe_set_debug_flags(fe_handle* h, int32_t flags) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
   if (flags < 0 || flags > 3) { snprintf(g_errbuf, sizeof g_errbuf, "flags must be in [0, 3]"); return FE_EINVAL; }
@@ -707,10 +714,7 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
   return FE_OK;
 }
 
-int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
-  if (!h || !q_xy || !chi_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle, q_xy or chi_dev is NULL"); return FE_EINVAL; }
-  if (nq < 1 || nq > kMaxQ || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, %d], hz finite", kMaxQ); return FE_EINVAL; }
-  for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
+static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = h->N, nb = h->nb, nbb = nb * nb;
   if (int rcd = check_device(h)) return rcd;
@@ -787,6 +791,39 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   fe_chi_finish_kernel<<<(nout + 255) / 256, 256, 0, st>>>(nout, (int)nchunk, 1.0 / ((double)N * (double)N), h->d_partial, chi_dev);
   FE_CUDA(cudaGetLastError());
   h->launches++;
+  return FE_OK;
+}
+
+// q on the k-grid?  (then E(k + q) is the unshifted band table read at a shifted index: no table of its own)
+static bool chi_q_on_grid(const double* q, int N) {
+  const double mx = q[0] * N / (2.0 * 3.14159265358979323846), my = q[1] * N / (2.0 * 3.14159265358979323846);
+  return fabs(mx - nearbyint(mx)) <= 1e-9 && fabs(my - nearbyint(my)) <= 1e-9 && fabs(mx) < 1e15 && fabs(my) < 1e15;
+}
+
+int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
+  if (!h || !q_xy || !chi_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle, q_xy or chi_dev is NULL"); return FE_EINVAL; }
+  if (nq < 1 || nq > kMaxQ || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, %d], hz finite", kMaxQ); return FE_EINVAL; }
+  for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
+  if (h->nb < 3) return chi_slice(h, q_xy, nq, hz, chi_dev, cuda_stream);
+  // Three-band model: every q OFF the k-grid needs a band table of its own (24 MB at N = 1024).  The q list is processed
+  // in consecutive slices that hold at most `maxoff` such q-values, so the table scratch stays below ~2 GB (chi_table_budget) whatever the
+  // size of the map (a 48 x 48 off-grid map would otherwise need 55 GB); slices reuse the scratch in stream order.
+  const double table_bytes = 3.0 * (double)h->N * (double)h->N * sizeof(double);
+  int maxoff = (int)fmin(1.0e9, h->chi_table_budget / table_bytes) - 1;
+  if (maxoff < 1) maxoff = 1;
+  const int nbb = h->nb * h->nb;
+  int q0 = 0;
+  while (q0 < nq) {
+    int q1 = q0, noff = 0;
+    while (q1 < nq) {
+      const int off = chi_q_on_grid(q_xy + 2 * q1, h->N) ? 0 : 1;
+      if (noff + off > maxoff) break;
+      noff += off; ++q1;
+    }
+    const int rc = chi_slice(h, q_xy + 2 * q0, q1 - q0, hz, chi_dev + (size_t)q0 * nbb, cuda_stream);
+    if (rc) return rc;
+    q0 = q1;
+  }
   return FE_OK;
 }
 

@@ -25,19 +25,24 @@ __device__ __forceinline__ ChiSide chi_side(double x, double neg_beta, const Mat
   ChiSide s;
   s.x = x; s.ax = fabs(x);
   const double t = s.ax * neg_beta;            // -|x|/T <= 0
-  s.u = exp_nonpos(t, tabs);                   // branch-free (fe_math.cuh); keeps its relative accuracy when tiny
-  const double em = t > -0.6931 ? expm1(t) : s.u - 1.0;   // u - 1 without cancellation for |x| << T (states on
-  s.opu = 1.0 + s.u;                                      // the Fermi surface): tanh(|x|/2T) = (1-u)/(1+u)
+  double em;                                   // u - 1 without cancellation for |x| << T (states on the Fermi surface):
+  exp_em1_nonpos(t, tabs, s.u, em);            // tanh(|x|/2T) = (1-u)/(1+u); branch-free (fe_math.cuh)
+  s.opu = 1.0 + s.u;
   s.th = -em * rcp_nr(s.opu);
   return s;
 }
 
-__device__ __forceinline__ double chi_pair_factor(const ChiSide& a, const ChiSide& b, double inv2T) {
+__device__ __forceinline__ double chi_pair_factor(const ChiSide& a, const ChiSide& b, double inv2T, const MathTabs& tabs) {
   if (a.x * b.x > 0.0) return (a.th + b.th) * rcp_nr(2.0 * (a.ax + b.ax));
   const double z = fabs(a.x + b.x) * inv2T;
   const double w = fmax(a.u, b.u);
   const double rz = rcp_nr(fmax(z, 1e-300));
-  const double E = z > 20.0 ? rz : (z == 0.0 ? 2.0 : -expm1(-2.0 * z) * rz);
+  double E = rz;                                           // z > 20: 1 - exp(-2z) = 1 to fp64 (most opposite-sign pairs at low T)
+  if (z <= 20.0) {
+    double e2, em;
+    exp_em1_nonpos(-2.0 * z, tabs, e2, em);                // em = exp(-2z) - 1: -> -2z for z -> 0; branch-free inside
+    E = z == 0.0 ? 2.0 : -em * rz;                         // (a select)
+  }
   return w * E * inv2T * rcp_nr(a.opu * b.opu);
 }
 
@@ -99,7 +104,7 @@ __global__ void __launch_bounds__(kThreads) fe_chi_kernel(ModelConsts mc, double
 #pragma unroll
     for (int e = 0; e < NB; ++e)
 #pragma unroll
-      for (int f = 0; f < NB; ++f) acc[e * NB + f] = fma(g2, chi_pair_factor(A[e], B[f], inv2T), acc[e * NB + f]);
+      for (int f = 0; f < NB; ++f) acc[e * NB + f] = fma(g2, chi_pair_factor(A[e], B[f], inv2T, tabs), acc[e * NB + f]);
   }
   __shared__ double red[NB * NB][kWarps];
 #pragma unroll

@@ -31,6 +31,7 @@ struct MathTabs {               // global copy; kernels stage the parts they use
 
 __device__ __forceinline__ double exp_nonpos(double x, const MathTabs&) { return exp(x); }
 __device__ __forceinline__ double log_1p_w(double w, const MathTabs&) { return log1p(w); }
+__device__ __forceinline__ void exp_em1_nonpos(double x, const MathTabs&, double& u, double& em) { u = exp(x); em = expm1(x); }
 
 #else
 
@@ -55,6 +56,31 @@ __device__ __forceinline__ double exp_nonpos(double x, const MathTabs& tb) {
   int k = n >> 6;                                // floor(n / 64) in [-1039, 0]
   k = max(k, -1000);
   return __hiloint2double(__double2hiint(y) + (k << 20), __double2loint(y));
+}
+
+// u = exp(x) and em = exp(x) - 1 for finite x <= 0, both without branches and em without cancellation.  Same reduction as
+// exp_nonpos: exp(x) = c (1 + p), c = 2^(n>>6) 2^((n&63)/64), p = exp(r) - 1, so  exp(x) - 1 = (c - 1) + c p.  c - 1 is an
+// exact subtraction (c in (0, 1]); for |x| < ln2/128 it is 0 and em = p keeps full relative accuracy (x -> 0: em -> x); else
+// |em| >= 5.4e-3 and the table value's rounding (2^-53) is 2e-14 of it.  Used by the pair-susceptibility kernel for
+// tanh(|x|/2T) = -em / (1 + u) of states near the Fermi level and for (1 - exp(-2z)) / z through its removable singularity.
+__device__ __forceinline__ void exp_em1_nonpos(double x, const MathTabs& tb, double& u, double& em) {
+  const double L2E64 = 92.33248261689366;        // 64/ln2
+  const double LN2_64 = 0.010830424696249145;    // ln2/64
+  const double MAGIC = 6755399441055744.0;       // 1.5 * 2^52
+  x = fmax(x, -720.0);
+  const double t = fma(x, L2E64, MAGIC);
+  const int n = __double2loint(t);
+  const double r = fma(t - MAGIC, -LN2_64, x);
+  double p = fma(r, 8.3333333333333332e-03, 4.1666666666666664e-02);
+  p = fma(p, r, 1.6666666666666666e-01);
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = p * r;                                     // exp(r) - 1
+  const double s = tb.exp2_j64[n & 63];
+  const int k = max(n >> 6, -1000);
+  const double c = __hiloint2double(__double2hiint(s) + (k << 20), __double2loint(s));
+  u = fma(c, p, c);
+  em = fma(c, p, c - 1.0);
 }
 
 // ln(1 + w), 0 <= w <= 3.   y = 1 + w in [1, 4]; idx = top 8 bits below the leading one of y (with exponent),

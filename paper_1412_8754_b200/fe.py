@@ -20,7 +20,8 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
                "fe_get_launch_count", "fe_get_slot_counts", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
-EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math"]
+EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math",
+                 "fe_set_chi_table_budget"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
 
@@ -78,6 +79,7 @@ def lib():
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
     L.fe_set_debug_flags.argtypes = [vp, C.c_int32]
     L.fe_set_coop_shape.argtypes = [vp, C.c_int32]
+    L.fe_set_chi_table_budget.argtypes = [vp, C.c_double]
     L.fe_coop_shape_info.argtypes = [C.c_int32, ip]
     L.fe_fp64_peak_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_float), dp, vp]
     L.fe_debug_math.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp]
@@ -197,6 +199,9 @@ class FreeEnergy:
 
     def set_coop_shape(self, shape=0):
         _check(lib().fe_set_coop_shape(self._h, int(shape)))
+
+    def set_chi_table_budget(self, nbytes):
+        _check(lib().fe_set_chi_table_budget(self._h, float(nbytes)))
 
     def set_debug_flags(self, flags):
         _check(lib().fe_set_debug_flags(self._h, int(flags)))

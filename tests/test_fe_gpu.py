@@ -270,6 +270,17 @@ def test_pair_susceptibility_degenerate_and_errors(fe, oracle):
     ref = oracle.pair_susceptibility(w3.params, 24, 0.01, qmix, 0.02)
     assert np.max(np.abs(chi - ref) / np.abs(ref).max(axis=(1, 2), keepdims=True)) < 2e-12
     assert np.max(np.abs(chi_b - chi) / np.abs(chi).max()) < 1e-14
+    # an off-grid map larger than the table scratch is worked through in slices of the q list: same numbers, bit for bit
+    qoff = np.vstack([qmix, qmix + 0.013, -qmix + 0.4])
+    with fe.FreeEnergy(w3.params, 24, 0.01) as F:
+        whole = F.pair_susceptibility(qoff, 0.02).cpu().numpy()
+        F.set_chi_table_budget(2.5 * 3 * 24 * 24 * 8)             # room for ONE off-grid table (+ the unshifted one) per slice
+        sliced = F.pair_susceptibility(qoff, 0.02).cpu().numpy()
+        F.set_chi_table_budget(0.0)                                # a slice always takes at least one off-grid q
+        sliced0 = F.pair_susceptibility(qoff, 0.02).cpu().numpy()
+    assert np.array_equal(whole, sliced) and np.array_equal(whole, sliced0)
+    refo = oracle.pair_susceptibility(w3.params, 24, 0.01, qoff, 0.02)
+    assert np.max(np.abs(whole - refo) / np.abs(refo).max(axis=(1, 2), keepdims=True)) < 2e-12
     with fe.FreeEnergy(p, 8, 0.1) as F:
         with pytest.raises(fe.FeError):
             F.pair_susceptibility([(np.nan, 0.0)], 0.0)
