@@ -79,7 +79,12 @@ struct CoopGeom {
   static constexpr int WH = TH * LH;           // block tile, h
   static constexpr int WD = TD * NTD;          // block tile, Delta
   static constexpr int PADB = LH > 1 ? 2 : 0;  // B rows of the LH thread rows are 2 doubles apart in banks
-  static constexpr int W = WD + LH * (TH + PADB);            // doubles per slot row
+  // A' part of a slot row: TD/2 blocks of 2 NTD doubles (the two values a thread fetches with one LDS.128 are adjacent).
+  // The blocks are SA = 2 NTD + 8 doubles apart: thread t STORES A'_t at ((t % TD) / 2) SA + (t / TD) 2 + (t & 1), so the 16
+  // lanes of a half-warp hit {0..7} and {SA..SA+7}, 16 distinct 8-byte banks (with SA = 2 NTD they collided two by two)
+  static constexpr int SA = 2 * NTD + (TD > 2 ? 8 : 0);
+  static constexpr int AW = (TD / 2 - 1) * SA + 2 * NTD;     // doubles of the A' part
+  static constexpr int W = AW + LH * (TH + PADB);            // doubles per slot row
   static constexpr int SLOTS = KB * NB;        // slots per sub-batch
   static constexpr int BUF_DOUBLES = SLOTS * W + SLOTS;      // values + one int2 {eref, flags} per slot
   static constexpr int DPAD = 16;              // room behind the A-dominated list: its neutral padding (< 8) + one prefetch round (8)
@@ -90,8 +95,8 @@ struct CoopGeom {
       sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT) + sizeof(int) * 2 * (NW + 2);
   // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
   // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
-  __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * (2 * NTD) + (jg / TD) * 2 + (jg & 1); }
-  __host__ __device__ static constexpr int posB(int ib) { return WD + ib + (ib / TH) * PADB; }
+  __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * SA + (jg / TD) * 2 + (jg & 1); }
+  __host__ __device__ static constexpr int posB(int ib) { return AW + ib + (ib / TH) * PADB; }
 };
 
 // m 2^(e - eref) for m in [0.997, 2.51); shifts below -1000 are clamped there (the value is then < 2^-500 of its
@@ -487,11 +492,11 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     const int* const ev = ev_s + par * SLOTS * W;
     const int2* const efs = reinterpret_cast<const int2*>(val + SLOTS * W);
     const double* const va0 = val + tdx * 2;                          // + sl W + p 2 NTD
-    const double* const vb0 = val + WD + thx * (TH + G::PADB);        // + sl W + i
+    const double* const vb0 = val + G::AW + thx * (TH + G::PADB);     // + sl W + i
     auto load_a = [&](double (&a)[TD], int sl) {
 #pragma unroll
       for (int pp = 0; pp < TD / 2; ++pp) {
-        const double2 v = *reinterpret_cast<const double2*>(va0 + sl * W + pp * 2 * G::NTD);
+        const double2 v = *reinterpret_cast<const double2*>(va0 + sl * W + pp * G::SA);
         a[2 * pp] = v.x; a[2 * pp + 1] = v.y;
       }
     };
@@ -569,7 +574,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
             if (c == NQ - 2) {
 #pragma unroll
               for (int pp = 0; pp < TD / 2; ++pp) {
-                const double2 v = *reinterpret_cast<const double2*>(pa + W + pp * 2 * G::NTD);
+                const double2 v = *reinterpret_cast<const double2*>(pa + W + pp * G::SA);
                 an[2 * pp] = v.x; an[2 * pp + 1] = v.y;
               }
             }
@@ -651,10 +656,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
             for (int j = 0; j < TD; ++j) accP[HC + i][j] *= (a[j] + b1[i]);
         } else if (flags & kCoopRobust) {
           const double* const vb = vb0 + sl * W;
-          const int* const eb = ev + WD + thx * (TH + G::PADB) + sl * W;
+          const int* const eb = ev + G::AW + thx * (TH + G::PADB) + sl * W;
 #pragma unroll
           for (int j = 0; j < TD; ++j) {
-            const int pa = sl * W + (j / 2) * (2 * G::NTD) + tdx * 2 + (j & 1);
+            const int pa = sl * W + (j / 2) * G::SA + tdx * 2 + (j & 1);
             const double mA = val[pa];
             const int eA = ev[pa];
 #pragma unroll
