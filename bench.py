@@ -576,7 +576,7 @@ def main():
             band_evals = be
             if args.mode in ("coop", "coop_eo"):
                 c = F.slot_counts()                     # device -> host read of four counters, outside the events
-                tot = sum(c.values()) - c["padding"]
+                tot = c["dense"] + c["a_dominated"] + c["b_dominated"]
                 slot_kinds[f"T={step_T[-1]:g}"] = {k: v / tot for k, v in c.items()}
     barrier()
     t_wall = time.perf_counter() - t_wall0

@@ -189,11 +189,12 @@ int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
 
 /* What the most recent TIMED cooperative k-sum launch (FE_EVAL_COOP / FE_EVAL_COOP_EO with fe_enable_timing on) was made
- * of: counts4 = {dense, A-dominated, B-dominated, padding} (k, band) slots, each counted once per block tile it was
- * classified for (a slot of a 64 x 128 block tile stands for 8192 (h, Delta) pairs).  Dense and padding slots run through
- * the pair products, dominated slots are summed without exponentials (FE_EVAL_COOP_EO; FE_EVAL_COOP has none).  HOST
- * doubles; call after synchronising the stream (the call copies four counters from the device).  FE_EINVAL if there is none. */
-int fe_get_slot_counts(fe_handle* h, double* counts4);
+ * of: counts5 = {dense, A-dominated (summed as square roots per Delta_j), B-dominated, padding, A-dominated (summed through
+ * the moment series)} (k, band) slots, each counted once per block tile it was classified for (a slot of a 64 x 128 block
+ * tile stands for 8192 (h, Delta) pairs).  Dense and padding slots run through the pair products, dominated slots are
+ * summed without exponentials (FE_EVAL_COOP_EO; FE_EVAL_COOP has none).  HOST doubles; call after synchronising the
+ * stream (the call copies five counters from the device).  FE_EINVAL if there is none. */
+int fe_get_slot_counts(fe_handle* h, double* counts5);
 
 /* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode actually
  * used, rows per k-chunk}; for FE_EVAL_COOP / FE_EVAL_COOP_EO: {WH, WD, ksplit, grid blocks, mode, k-points per chunk};

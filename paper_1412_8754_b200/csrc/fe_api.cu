@@ -98,7 +98,7 @@ struct fe_handle {
   bool timing_valid = false;
   double last_band_evals = 0;
   int32_t last_info[6] = {0, 0, 0, 0, 0, 0};   // th, td, ksplit, grid, mode, rows_per_chunk
-  unsigned long long* d_kinds = nullptr;       // 4 slot-kind counters of the most recent timed K1c launch
+  unsigned long long* d_kinds = nullptr;       // 5 slot-kind counters of the most recent timed K1c launch
   bool kinds_valid = false;
   int64_t launches = 0;
 };
@@ -534,8 +534,8 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     CP.kind_counts = nullptr;
     h->kinds_valid = false;
     if (h->timing) {
-      if (!h->d_kinds) FE_CUDA(cudaMalloc((void**)&h->d_kinds, 4 * sizeof(unsigned long long)));
-      FE_CUDA(cudaMemsetAsync(h->d_kinds, 0, 4 * sizeof(unsigned long long), st));
+      if (!h->d_kinds) FE_CUDA(cudaMalloc((void**)&h->d_kinds, 5 * sizeof(unsigned long long)));
+      FE_CUDA(cudaMemsetAsync(h->d_kinds, 0, 5 * sizeof(unsigned long long), st));
       CP.kind_counts = h->d_kinds;
       h->kinds_valid = true;
     }
@@ -960,12 +960,12 @@ int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
   return FE_OK;
 }
 
-int fe_get_slot_counts(fe_handle* h, double* counts4) {
-  if (!h || !counts4) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+int fe_get_slot_counts(fe_handle* h, double* counts5) {
+  if (!h || !counts5) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
   if (!h->kinds_valid || !h->d_kinds) { snprintf(g_errbuf, sizeof g_errbuf, "no timed cooperative k-sum launch recorded"); return FE_EINVAL; }
-  unsigned long long c[4];
+  unsigned long long c[5];
   FE_CUDA(cudaMemcpy(c, h->d_kinds, sizeof c, cudaMemcpyDeviceToHost));
-  for (int i = 0; i < 4; ++i) counts4[i] = (double)c[i];
+  for (int i = 0; i < 5; ++i) counts5[i] = (double)c[i];
   return FE_OK;
 }
 

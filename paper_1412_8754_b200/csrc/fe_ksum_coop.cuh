@@ -52,8 +52,8 @@ struct CoopParams {
   const MathTabs* tabs;
   const double* etab;                  // NB == 3 only: [1 + nq][3][N*N] band tables, y = 0: E(k), 1 + iq: E(k - q)
   double* partial;                     // [ksplit][nq*nh*nd]
-  unsigned long long* kind_counts;     // NULL, or 4 device counters {dense, A-dominated, B-dominated, padding} slots, summed
-                                       // over all blocks of the launch (fe_enable_timing; block-tile slots of WH x WD pairs)
+  unsigned long long* kind_counts;     // NULL, or 5 device counters {dense, A-dominated (list), B-dominated, padding, A-dominated
+                                       // (moment series)} slots, summed over all blocks of the launch (fe_enable_timing)
 };
 
 struct __align__(16) CoopHdr {         // one per (k, band) slot
@@ -70,6 +70,17 @@ constexpr int kCoopSkip = 1, kCoopRobust = 2;
 // worst case of a pair sitting exactly at the threshold (pairs are spread over thousands of T beyond it, so the sum of what
 // is neglected is orders of magnitude smaller still).  Same bound for the B-dominated slots (T ln Z_ij = |d_i|).
 constexpr int kDomGap = 50;
+// A-dominated slots whose radicand is dominated by s^2 over the whole tile, eps_j = Delta_j^2 g / s^2 <= 1/16, are not even
+// square-rooted per Delta_j:  R_j = |s| sqrt(1 + eps_j) = |s| sum_m c_m eps_j^m  (binomial series, c_m = binom(1/2, m)), so
+//     sum_k R_j(k) = sum_m c_m Delta_j^(2m) M_m,      M_m = sum_k |s_k| x_k^m,   x_k = g_k / s_k^2,
+// and the thread that owns k in P0 adds its kMomN moments once for ALL Delta_j of the tile (2 FP64 instructions per order
+// instead of 7 per Delta_j); the polynomial in Delta_j^2 is evaluated once per block.  Truncation after m = kMomN - 1 = 12:
+// |c_13| (1/16)^13 / (1 - 1/16) < 2^-59 relative to R_j.  On config 4, 95 - 98 % of the A-dominated slots qualify.
+constexpr int kMomN = 13;
+constexpr double kMomEps = 0.0625;
+__device__ __constant__ const double kMomC[kMomN] = {1.0, 0.5, -0.125, 0.0625, -5.0 / 128, 7.0 / 256, -21.0 / 1024, 33.0 / 2048,
+                                                      -429.0 / 32768, 715.0 / 65536, -2431.0 / 262144, 4199.0 / 524288,
+                                                      -29393.0 / 4194304};
 
 template <int TH, int TD, int LH, int NW, int KB, int NB>
 struct CoopGeom {
@@ -92,7 +103,7 @@ struct CoopGeom {
                                                // sub-batches), B- then A-dominated slots at the back
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
-      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT) + sizeof(int) * 2 * (NW + 2);
+      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT + kMomN * NT + kMomN * NW) + sizeof(int) * 2 * (NW + 2);
   // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
   // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
   __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * SA + (jg / TD) * 2 + (jg & 1); }
@@ -122,7 +133,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   double* const rng_s = h_s + WH;                                                    // hmin hmax d2min d2max (+pad)
   double* const accR_s = rng_s + 8;                                                  // [WD] sums of R_j over A-dominated slots
   double* const accB_s = accR_s + WD;                                                // [NT / WH][WH] sums of |d_i| over B-dominated slots
-  int* const ev_s = reinterpret_cast<int*>(accB_s + NT);                             // 2 x [SLOTS][W] (robust slots)
+  double* const mom_s = accB_s + NT;                                                 // [kMomN][NT] moments M_m, one column per thread
+  double* const momred_s = mom_s + kMomN * NT;                                       // [kMomN][NW] their per-warp sums
+  int* const ev_s = reinterpret_cast<int*>(momred_s + kMomN * NW);                   // 2 x [SLOTS][W] (robust slots)
   int* const accE_s = ev_s + 2 * SLOTS * W;                                          // [TH*TD][NT]
   int* const scan_s = accE_s + TH * TD * NT;                                         // [2][NW + 2] compaction scan
 
@@ -142,6 +155,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   for (int i = tid; i < WH; i += NT) h_s[i] = P.h[min(th * WH + i, P.nh - 1)];
   for (int i = tid; i < WD; i += NT) accR_s[i] = 0.0;
   accB_s[tid] = 0.0;
+#pragma unroll
+  for (int m = 0; m < kMomN; ++m) mom_s[m * NT + tid] = 0.0;
   int* const myE = accE_s + tid;
 #pragma unroll
   for (int pq = 0; pq < TH * TD; ++pq) myE[pq * NT] = 0;
@@ -209,6 +224,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     CoopHdr hd[NB];
     int kind[NB];                                            // 0 dropped, 1 dense, 2 A-dominated, 3 B-dominated
     int cnt = 0;                                             // dense | A-dominated << 10 | B-dominated << 20 (each <= NT NB < 1024)
+    int nser = 0;                                            // A-dominated slots of this thread taken by the moment series
 #pragma unroll
     for (int e = 0; e < NB; ++e) {
       const double s = fma(0.5, Ek[e] + Eq[e], -P.mc.mu);    // (a + b)/2                  (S3)
@@ -233,6 +249,17 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       if (early_out && !force_robust && eAlo - eBhi >= kDomGap) kind[e] = 2;
       if (early_out && !force_robust && eBlo - eAhi >= kDomGap) kind[e] = 3;
       if (!valid || !((P.mc.band_mask >> e) & 1)) kind[e] = 0;
+      if (kind[e] == 2 && d2max * g2 <= kMomEps * s2) {       // A-dominated and eps_j <= 1/16 for every Delta_j of the tile:
+        kind[e] = 4;                                         // its R_j enter through the moments, not the list (kMomN)
+        const double x = g2 * rcp_nr(s2);
+        double t = fabs(s);
+#pragma unroll
+        for (int m = 0; m < kMomN; ++m) {
+          mom_s[m * NT + tid] += t;                          // (this thread's own column)
+          t *= x;
+        }
+        ++nser;
+      }
       any_robust |= kind[e] == 1 && robust;
       cnt += kind[e] == 1 ? 1 : (kind[e] == 2 ? (1 << 10) : (kind[e] == 3 ? (1 << 20) : 0));
     }
@@ -281,6 +308,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       if (ndom) atomicAdd(P.kind_counts + 1, (unsigned long long)ndom);
       if (ndomB) atomicAdd(P.kind_counts + 2, (unsigned long long)ndomB);
       if (nsub * SLOTS - ndense) atomicAdd(P.kind_counts + 3, (unsigned long long)(nsub * SLOTS - ndense));
+    }
+    if (P.kind_counts != nullptr) {                          // (uniform branch) series slots: one atomic per warp
+      const unsigned ws = __reduce_add_sync(0xffffffffu, (unsigned)nser);
+      if (lane == 0 && ws) atomicAdd(P.kind_counts + 4, (unsigned long long)ws);
     }
     // A-dominated slots: T ln Z_ij = R_j for the whole tile (kDomGap); this thread owns Delta_j, j = tid + r NT
     if (ndom > 0) {
@@ -677,6 +708,30 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     }
     cur_robust = nxt_robust; cur_exists = nxt_exists; j = jn; nsub = nsub_n; par ^= 1;
     __syncthreads();     // buffer `par ^ 1` may be rewritten (by P1 of the sub-batch after next), buffer `par` is complete
+  }
+
+  // Moment series of the A-dominated slots (kMomN): column sums in a fixed order (shuffle tree per warp, then the warps in
+  // index order), then sum_m c_m Delta_j^(2m) M_m per Delta_j of the tile (Horner in Delta_j^2), added to the list sums.
+  if (early_out) {
+#pragma unroll
+    for (int m = 0; m < kMomN; ++m) {
+      const double v = warp_sum(mom_s[m * NT + tid]);
+      if (lane == 0) momred_s[m * NW + warp] = v;
+    }
+    __syncthreads();
+    for (int jg = tid; jg < WD; jg += NT) {
+      const double d2 = d2_s[jg];
+      double poly = 0.0;
+#pragma unroll
+      for (int m = kMomN - 1; m >= 0; --m) {
+        double M = momred_s[m * NW];
+#pragma unroll
+        for (int w = 1; w < NW; ++w) M += momred_s[m * NW + w];
+        poly = fma(poly, d2, kMomC[m] * M);
+      }
+      accR_s[jg] += poly;
+    }
+    __syncthreads();
   }
 
   // P_ij = T (ln2 * exponent sum + ln accP_ij); every thread owns its (h, Delta) pairs for the whole chunk

@@ -221,10 +221,11 @@ class FreeEnergy:
         return dict(th=a[0], td=a[1], ksplit=a[2], grid=a[3], mode=a[4], rows_per_chunk=a[5])
 
     def slot_counts(self):
-        """{dense, a_dominated, b_dominated, padding} slot counts of the most recent timed cooperative k-sum launch."""
-        a = (C.c_double * 4)()
+        """{dense, a_dominated (= list + series), a_series, b_dominated, padding} slot counts of the most recent timed
+        cooperative k-sum launch."""
+        a = (C.c_double * 5)()
         _check(lib().fe_get_slot_counts(self._h, a))
-        return dict(dense=a[0], a_dominated=a[1], b_dominated=a[2], padding=a[3])
+        return dict(dense=a[0], a_dominated=a[1] + a[4], a_series=a[4], b_dominated=a[2], padding=a[3])
 
     def launch_count(self):
         n = C.c_int64()
