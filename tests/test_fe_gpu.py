@@ -492,6 +492,35 @@ def test_full_size_properties_in_bench_launch_configuration(fe):
             assert bool(torch.isfinite(a).all())
 
 
+def test_slot_counters_and_moment_series(fe, oracle):
+    """fe_get_slot_counts: every (k, band, block tile) slot of a timed launch is classified exactly once; the dense variant has
+    no dominated slots; at low T most A-dominated slots go through the moment series (Delta^2 g <= s^2 / 16 over the tile),
+    and a grid with large Delta (eps > 1/16 near the Fermi surface) uses both the series and the square-root list."""
+    import torch
+    for w, T in ((W.config(2), 0.001), (W.interior_minimum(N=96, U=5.0, T=0.002, nq=2, nh=64, nd=128), 0.002),
+                 (W.Workload("big_delta", W.model_params(U=4.0), 64, (0.002,), np.array([[0.2, 0.1]]), np.linspace(0, 0.1, 64),
+                             np.linspace(0.0, 3.0, 128)), 0.002)):
+        ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        for mode in (fe.EVAL_COOP_EO, fe.EVAL_COOP):
+            with fe.FreeEnergy(w.params, w.N, T) as F:
+                F.set_eval_mode(mode)
+                F.set_coop_shape(1)
+                F.enable_timing(True)
+                om = F.omega_grid(w.q, w.h, w.delta)
+                torch.cuda.synchronize()
+                c = F.slot_counts()
+                info = F.last_launch_info()
+            assert max_rel(om.cpu().numpy(), ref) < RTOL
+            tiles = w.nq * -(-w.nh // info["th"]) * -(-w.nd // info["td"])
+            assert c["dense"] + c["a_dominated"] + c["b_dominated"] == w.N * w.N * w.nbands * tiles
+            if mode == fe.EVAL_COOP:
+                assert c["a_dominated"] == 0 and c["b_dominated"] == 0 and c["a_series"] == 0
+            else:
+                assert c["a_dominated"] > 0.5 * c["dense"] and 0 < c["a_series"] <= c["a_dominated"]
+                if w.name == "big_delta":
+                    assert c["a_series"] < c["a_dominated"]          # some dominated slots have eps > 1/16: list path
+
+
 def test_factored_extreme_spreads(fe, oracle):
     """h list spanning many temperatures inside one tile (no recurrence, large exponent spread) and a tiny T where
     the spread exceeds 900 binades (robust path taken on its own)."""
