@@ -39,7 +39,7 @@ constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 // KB k-points per shared-memory sub-batch, MINB resident blocks per SM.  Block tile = (TH LH) x (TD NW 32/LH).
 struct CoopShape { int th, td, lh, nw, kb, minb; };
 constexpr CoopShape kCoopShapes[] = {{16, 4, 4, 4, 4, 2}, {16, 4, 1, 4, 2, 2}, {8, 4, 4, 4, 4, 3}, {8, 4, 1, 4, 2, 2},
-                                     {16, 4, 4, 4, 2, 2}};   // last: shape 0 with half the sub-batch (early-out mode)
+                                     {16, 4, 2, 4, 2, 2}};   // last: 32 x 256 block tile (one- and two-band models)
 constexpr int kNumCoopShapes = sizeof(kCoopShapes) / sizeof(kCoopShapes[0]);
 constexpr int kStageSlots = 4;
 constexpr int kSChunksMax = 128;
@@ -270,10 +270,10 @@ double coop_shape_cost(const CoopShape& s) {
   return (pair + expo) / pair * (s.th * s.td >= 64 ? 1.0 : 1.08);
 }
 
-int choose_coop_shape(const fe_handle* h, int nh, int nd, bool early_out) {
+int choose_coop_shape(const fe_handle* h, const double* h_list, int nh, int nd, bool early_out) {
   if (h->coop_shape > 0) return h->coop_shape - 1;
   int best = 0; double best_cost = 1e300;
-  for (int t = 0; t < 4; ++t) {
+  for (int t = 0; t < kNumCoopShapes; ++t) {
     const CoopShape& s = kCoopShapes[t];
     if (h->nb == 3 && s.lh != 4) continue;
     const int wh = s.th * s.lh, wd = s.td * s.nw * (32 / s.lh);
@@ -281,9 +281,20 @@ int choose_coop_shape(const fe_handle* h, int nh, int nd, bool early_out) {
     const double cost = padded * coop_shape_cost(s);
     if (cost < best_cost * (1.0 - 1e-12)) { best_cost = cost; best = t; }
   }
-  // early-out mode pads the compacted dense slots of every group to whole sub-batches: the half-size sub-batch of
-  // shape 4 wastes less (measured + 1.5 % on config 4; the dense variant is 3.5 % faster with the full sub-batch)
-  if (early_out && best == 0) best = 4;
+  // Early-out mode classifies a (k, band) slot for a whole block tile, so a tile that is narrower along h leaves fewer
+  // slots dense when the dominance window kDomGap T ln2 is small against the h range of the tile; the 32 x 256 tile pays
+  // ~12 % more per dense slot (WD + WH = 288 instead of 192 exponentials per 8192 pairs).  Measured on config 4 (h range
+  // 0.3 per 64 values; launches in ms, 64 x 128 vs 32 x 256): T = 0.0005 63.1 / 46.8, 0.001 58.6 / 47.6, 0.002 56.4 / 52.7,
+  // 0.004 63.7 / 62.7, 0.006 70.4 / 72.3, 0.01 83.6 / 88.6, 0.02 117.6 / 128.9: the narrow tile wins below window / range ~ 0.5.
+  if (early_out && best == 0 && h->nb < 3 && nh > 32) {
+    double range = 0.0;
+    for (int t0 = 0; t0 < nh; t0 += 64) {
+      double lo = h_list[t0], hi = h_list[t0];
+      for (int i = t0; i < nh && i < t0 + 64; ++i) { lo = fmin(lo, h_list[i]); hi = fmax(hi, h_list[i]); }
+      range = fmax(range, hi - lo);
+    }
+    if ((double)kDomGap * h->T * 0.6931471805599453 < 0.5 * range) best = 4;
+  }
   return best;
 }
 
@@ -325,7 +336,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
   if (h->nb == 3 && mode != FE_EVAL_COOP) {
     snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND supports FE_EVAL_COOP / FE_EVAL_COOP_EO only"); return FE_EINVAL; }
   if (mode == FE_EVAL_COOP) {
-    cshape = choose_coop_shape(h, nh, nd, early_out);
+    cshape = choose_coop_shape(h, h_list, nh, nd, early_out);
     if (h->nb == 3 && kCoopShapes[cshape].lh != 4) {
       snprintf(g_errbuf, sizeof g_errbuf, "FE_MODEL_THREE_BAND needs a coop shape with 4 lanes along h"); return FE_EINVAL; }
     if (h->coop_shape == 0 && h->nb < 3) {

@@ -99,8 +99,8 @@ struct CoopGeom {
   static constexpr int SLOTS = KB * NB;        // slots per sub-batch
   static constexpr int BUF_DOUBLES = SLOTS * W + SLOTS;      // values + one int2 {eref, flags} per slot
   static constexpr int DPAD = 16;              // room behind the A-dominated list: its neutral padding (< 8) + one prefetch round (8)
-  static constexpr int HTOT = NT * NB + SLOTS + DPAD;   // header array: dense slots compacted at the front (padded to whole
-                                               // sub-batches), B- then A-dominated slots at the back
+  static constexpr int HTOT = NT * NB + 2 * SLOTS + DPAD;   // header array: dense slots compacted at the front (behind the < SLOTS
+                                               // slots carried over from the previous group), B- then A-dominated slots at the back
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
       sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT + kMomN * NT + kMomN * NW) + sizeof(int) * 2 * (NW + 2);
@@ -193,13 +193,21 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 
   // ---------------- P0: one k-point per thread -> NB slot headers (for NT consecutive k-points) ----------------
   // The NT*NB slots of a group are sorted into three kinds.  DENSE slots are compacted, in k order, to the front of
-  // hdr_s and padded with neutral skip slots to whole sub-batches of SLOTS; A-DOMINATED slots (early-out mode only)
+  // hdr_s, behind the `nleft` (< SLOTS) dense slots the previous groups left over; only whole sub-batches of SLOTS are
+  // handed to P1 / P2, the remainder is carried into the next group (the last group of the chunk pads it with neutral
+  // skip slots: one padded sub-batch per chunk instead of one per group); A-DOMINATED slots (early-out mode only)
   // go to the back of hdr_s and are summed right here, sum_k R_j per Delta_j of the block tile, by the thread that
   // owns Delta_j (no exponential, no pair work), B-DOMINATED slots likewise as sum_k |d0 - h_i| per h_i; skip slots (k past the chunk end, masked band) are dropped.
   // Returns (to every thread, through the barriers) the number of dense sub-batches of the group and whether any
   // of its dense slots needs the robust path.
   const bool early_out = P.early_out != 0;
-  auto p0 = [&](int superbatch, int& nsub_out) -> bool {
+  // dense slots carried over: count (< SLOTS) | may be robust << 8 | position in hdr_s << 9 (one register across the main loop)
+  int carry_state = 0;
+  auto p0 = [&](int superbatch, bool last_group, int& nsub_out) -> bool {
+    const int nleft = carry_state & 0xff;
+    const bool left_robust = (carry_state >> 8) & 1;
+    CoopHdr carried;                                         // thread tid < nleft moves carried slot tid to the front
+    if (tid < nleft) carried = hdr_s[(carry_state >> 9) + tid];
     const unsigned long long kidx = kbeg + (unsigned long long)superbatch * NT + tid;
     const bool valid = kidx < kend;
     const unsigned long long kk = valid ? kidx : kbeg;
@@ -280,9 +288,11 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       total += v;
     }
     const int ndense = total & 0x3ff, ndom = (total >> 10) & 0x3ff, ndomB = total >> 20;
-    const int nsub = (ndense + SLOTS - 1) / SLOTS;
+    const int nfront = nleft + ndense;                       // dense slots waiting at the front of hdr_s
+    const int nsub = last_group ? (nfront + SLOTS - 1) / SLOTS : nfront / SLOTS;
     const int off = base + incl - cnt;                       // exclusive prefix of the three counts
-    int pd = off & 0x3ff;                                    // first dense position of this thread
+    int pd = nleft + (off & 0x3ff);                          // first dense position of this thread
+    if (tid < nleft) hdr_s[tid] = carried;                   // (every thread has read its carried slot before the scan's barrier)
     constexpr int DEND = G::HTOT - G::DPAD;                  // end of the A-dominated list
     int pm = DEND - ndom + ((off >> 10) & 0x3ff);            // first A-dominated position (back of the array)
     int pb = DEND - ndom - ndomB + (off >> 20);              // first B-dominated position (just before them)
@@ -292,22 +302,27 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       else if (kind[e] == 2) hdr_s[pm++] = hd[e];
       else if (kind[e] == 3) hdr_s[pb++] = hd[e];
     }
-    if (tid < nsub * SLOTS - ndense) {                       // neutral padding of the last sub-batch
+    const int npad = last_group ? nsub * SLOTS - nfront : 0;
+    if (tid < npad) {                                        // neutral padding of the chunk's last sub-batch
       CoopHdr z;
       z.s2 = 1.0; z.g2 = 0.0; z.d0 = 0.0; z.eref = 0; z.flags = kCoopSkip;
-      hdr_s[ndense + tid] = z;
+      hdr_s[nfront + tid] = z;
     }
     if (tid < ((8 - (ndom & 7)) & 7)) {                      // the A-dominated list is summed 8 entries at a time: pad it with
       CoopHdr z;                                             // entries that add sqrt(1e-300) = 1e-150 to a sum of O(1) terms
       z.s2 = 1e-300; z.g2 = 0.0; z.d0 = 0.0; z.eref = 0; z.flags = kCoopSkip;
       hdr_s[DEND + tid] = z;
     }
-    const bool rob = __syncthreads_or(any_robust) != 0;
+    const bool rob = (__syncthreads_or(any_robust) != 0) || left_robust;
+    {
+      const int nl = last_group ? 0 : nfront - nsub * SLOTS;
+      carry_state = nl | ((rob && nl > 0) ? 0x100 : 0) | ((nsub * SLOTS) << 9);
+    }
     if (P.kind_counts != nullptr && tid == 0) {              // diagnostics only (fe_enable_timing): what the launch was made of
       if (ndense) atomicAdd(P.kind_counts + 0, (unsigned long long)ndense);
       if (ndom) atomicAdd(P.kind_counts + 1, (unsigned long long)ndom);
       if (ndomB) atomicAdd(P.kind_counts + 2, (unsigned long long)ndomB);
-      if (nsub * SLOTS - ndense) atomicAdd(P.kind_counts + 3, (unsigned long long)(nsub * SLOTS - ndense));
+      if (npad) atomicAdd(P.kind_counts + 3, (unsigned long long)npad);
     }
     if (P.kind_counts != nullptr) {                          // (uniform branch) series slots: one atomic per warp
       const unsigned ws = __reduce_add_sync(0xffffffffu, (unsigned)nser);
@@ -450,7 +465,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   auto next_group = [&](int& nsub_out, bool& robust_out) -> bool {
     while (group_next < ngroups) {
       int ns = 0;
-      const bool rob = p0(group_next++, ns);
+      const bool last = group_next + 1 == ngroups;
+      const bool rob = p0(group_next++, last, ns);
       if (ns > 0) { nsub_out = ns; robust_out = rob; return true; }
     }
     return false;

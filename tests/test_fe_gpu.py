@@ -341,6 +341,25 @@ def test_coop_early_out_extremes(fe, oracle):
     assert np.array_equal(a, b)
 
 
+def test_early_out_block_tile_follows_the_dominance_window(fe, oracle):
+    """Early-out mode picks the block tile from the ratio of the dominance window (kDomGap T ln2) to the h range of a tile:
+    32 x 256 when the window is narrow (fewer slots stay dense), 64 x 128 otherwise; both agree with the oracle, and the
+    remainder of a group's dense slots is carried into the next group (one chunk: target_blocks = 1)."""
+    import torch
+    w = W.interior_minimum(N=48, U=5.0, T=0.001, nq=2, nh=64, nd=256)
+    assert float(w.h.max() - w.h.min()) > 0.1
+    for T, tile in ((0.0005, (32, 256)), (0.05, (64, 128))):
+        for tb in (0, 1):
+            ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+            with fe.FreeEnergy(w.params, w.N, T) as F:
+                F.set_tuning(0, tb)
+                om = F.omega_grid(w.q, w.h, w.delta)
+                torch.cuda.synchronize()
+                info = F.last_launch_info()
+            assert info["mode"] == fe.EVAL_COOP_EO and (info["th"], info["td"]) == tile, info
+            assert max_rel(om.cpu().numpy(), ref) < 1e-12
+
+
 # ---- single-precision builds and screening + verification (SURVEY.md 8f-2, PAPER.md:190-198) ----
 EPS32 = float(np.finfo(np.float32).eps)
 
