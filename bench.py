@@ -558,6 +558,7 @@ def main():
     launches0 = F.launch_count()
     step_ms, ksum_ms, step_T, band_evals = [], [], [], 0.0
     slot_kinds = {}                                     # per temperature: what the timed launches were made of (in-run counters)
+    tiles_by_T = {}                                     # per temperature: block tile the library chose
     res = None
     barrier()
     t_wall0 = time.perf_counter()
@@ -574,6 +575,8 @@ def main():
             ms, be = F.last_ksum()
             ksum_ms.append(ms)
             band_evals = be
+            li = F.last_launch_info()
+            tiles_by_T[f"T={step_T[-1]:g}"] = f"{li['th']}x{li['td']}"
             if args.mode in ("coop", "coop_eo"):
                 c = F.slot_counts()                     # device -> host read of four counters, outside the events
                 tot = c["dense"] + c["a_dominated"] + c["b_dominated"]
@@ -613,6 +616,7 @@ def main():
         dinfo = F.last_launch_info()
         dense = {"eval_mode": "coop", "steps": len(d_ms), "value": evals_rank_step * len(d_ms) / (sum(d_ms) * 1e-3), "unit": UNIT,
                  "ms_per_step": sum(d_ms) / len(d_ms), "ms_per_step_median": statistics.median(d_ms), "ksum_ms": sum(dk_ms) / len(dk_ms),
+                 "ksum_ms_steps": [[f"T={t:g}", round(x, 3)] for t, x in zip(d_T, dk_ms)],
                  "tile": [dinfo["th"], dinfo["td"]], "grid": dinfo["grid"]}
         droof = roofline_base("dense", 1.0)
         dcounts, dstatus = kernel_counts(f"omega/coop/{w.name}/q{nq_step}", "fe_ksum", hashes)
@@ -621,6 +625,33 @@ def main():
             if k in droof:
                 dense["roofline_" + k] = droof[k]
         F.set_eval_mode(mode)
+
+    # ---- the opt-in mirror-symmetry variant (fe_set_symmetry), timed beside the headline and NEVER folded
+    #      into `value`: when every q of the step is invariant under a lattice mirror (config 4: q on the diagonal) the
+    #      k-sum visits one k-point per orbit.  `value` counts the nominal N x N k-points, as the headline does. ----
+    symv = None
+    if args.mode == "coop_eo" and not args.no_dense and nq_rank and w.nbands < 3:
+        F.set_symmetry(True)
+        one_step(0); one_step(1)
+        barrier()
+        s_ms, s_sym = [], 0
+        for s in range(2 * len(temps)):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            one_step(s)
+            e1.record(stream)
+            e1.synchronize()
+            s_ms.append(e0.elapsed_time(e1))
+            s_sym = F.last_symmetry()
+        barrier()
+        F.set_symmetry(False)
+        if s_sym:
+            symv = {"what": "fe_set_symmetry(1): k-sum over one k-point per mirror orbit (weights 2 / 1); same Omega to rounding, "
+                            "parity-tested against the oracle; reported separately, not the headline",
+                    "mirror": {1: "k_y -> -k_y", 2: "k_x -> -k_x", 3: "k_x <-> k_y"}[s_sym], "steps": len(s_ms),
+                    "value": evals_rank_step * len(s_ms) / (sum(s_ms) * 1e-3), "unit": UNIT + " (nominal N x N k-points)",
+                    "ms_per_step": sum(s_ms) / len(s_ms), "ms_per_step_median": statistics.median(s_ms)}
 
     # ---- e2e: host buffers through fe_scan_host (pinned), copies inside the timed region; N > 1: + gather of the minima ----
     pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()    # noqa: E731
@@ -676,7 +707,8 @@ def main():
     # Primary roofline = FP64-pipe lane-instructions/s: a DADD or DMUL occupies an FP64 lane for a cycle exactly like a
     # DFMA, and the kernel's pair update acc *= (A + B) has no fused form, so instructions (not flops, which count a
     # DFMA twice) measure how busy the bounding unit is; frac_tflops (DFMA = 2) is printed beside it.
-    roofline = roofline_base(f"k-sum kernel ({args.mode}, tile {info['th']}x{info['td']}, grid {info['grid']} x {info['block']})", dfma_rate)
+    tile_desc = ", ".join(f"{k}: {v}" for k, v in sorted(tiles_by_T.items())) if len(set(tiles_by_T.values())) > 1 else f"{info['th']}x{info['td']}"
+    roofline = roofline_base(f"k-sum kernel ({args.mode}, block tile {tile_desc}, grid {info['grid']} x {info['block']})", dfma_rate)
     roofline.update({"avg_launch_ms": k_ms, "median_launch_ms": statistics.median(ksum_ms), "band_evals_per_launch": band_evals,
                      "kernel_share_of_step": sum(ksum_ms) / total_ms})
     if slot_kinds:
@@ -705,7 +737,7 @@ def main():
                     "steps": e2e_steps, "api": "fe_scan_host (host buffers in/out, synchronous)" +
                     (" + all_gather of the minima" if world > 1 else "")},
             "gpu_launches": launches, "wall_s_timed_region": t_wall, "clocks": clocks, "source_hash": hashes[0],
-            "roofline": roofline, "dense_variant": dense, "cpu_baseline": cpu, "result_check": idx_check}
+            "roofline": roofline, "dense_variant": dense, "symmetric_variant": symv, "cpu_baseline": cpu, "result_check": idx_check}
     if sp_mode:
         line["verified_per_step"] = verified[-args.steps:]
     print(json.dumps(line), flush=True)

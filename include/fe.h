@@ -53,8 +53,8 @@ extern "C" {
 
 /* ---- evaluation mode of the k-sum kernel (fe_set_eval_mode); both compute the same sums ----
  * COOP_EO : default.  The block-cooperative factored kernel with a block-uniform early-out: a (k, band) slot whose
- *           2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^48 over the whole block tile contributes
- *           T ln Z_ij = R_j (what is neglected is below half an ulp of the term), so it needs no pair products; the
+ *           2cosh(R_j/T) exceeds 2cosh(|d_i|/T) by more than 2^42 over the whole block tile contributes
+ *           T ln Z_ij = R_j (what is neglected is below 5.1e-15 of the term and one-signed), so it needs no pair products; the
  *           other slots are compacted and run through the dense pipeline.  Same results to ~1e-15 relative; several
  *           times fewer FP64 instructions at low T.
  * COOP    : the dense variant (every pair of every slot is multiplied out).  Uses 2cosh(d/T) + 2cosh(R/T) =
@@ -93,6 +93,18 @@ int fe_set_temperature(fe_handle* h, double T);
 /* Select FE_EVAL_COOP_EO (default) or FE_EVAL_COOP (or one of the cross-check modes of fe_debug.h) for subsequent
  * fe_omega_grid calls.  Unknown mode: FE_EINVAL. */
 int fe_set_eval_mode(fe_handle* h, int32_t mode);
+
+/* Opt-in mirror-symmetry reduction of the k-sum (default off).  The paper notes that symmetries of the dispersion can
+ * shorten Algorithm 1 (E(-k) = E(k) for q = 0, scans along specific q directions).  When on,
+ * every fe_omega_grid call whose q list is invariant, element by element and compared exactly, under one mirror M of the
+ * square lattice -- k_x <-> k_y (all q_x == q_y), k_y -> -k_y (all q_y == 0) or k_x -> -k_x (all q_x == 0) -- sums only
+ * the k-points with M k "above" k with weight 2 and the fixed points of M with weight 1: E_k, E_{k-q} and eta_k are the same
+ * at k and M k, so the terms are equal and half of the zone is visited.  Mathematically the same Omega; the summation order
+ * differs, so the result differs from the full-zone sum by rounding (~1e-15 relative).  One- and two-band models with the
+ * cooperative kernel (FE_EVAL_COOP / FE_EVAL_COOP_EO); other calls ignore the setting.  fe_get_last_symmetry reports
+ * what the most recent fe_omega_grid launch used: 0 none, 1 k_y -> -k_y, 2 k_x -> -k_x, 3 k_x <-> k_y.            */
+int fe_set_symmetry(fe_handle* h, int32_t on);
+int fe_get_last_symmetry(fe_handle* h, int32_t* sym);
 
 /* Omega on the full grid  (steps S1-S9 of DESIGN.md: k generation, dispersion A.1-A.4, Eq. 4, Eq. 5,
  * deterministic two-stage k-sum; Algorithm 1 lines 1-5, Algorithm 2).

@@ -43,6 +43,12 @@ int fe_set_debug_flags(fe_handle* h, int32_t flags);
  * a slice always holds at least one off-grid q).  Lets tests force the slicing on small grids.  Results do not depend on it. */
 int fe_set_chi_table_budget(fe_handle* h, double bytes);
 
+/* Host-only test hook for fe_set_symmetry: the symmetry-reduced k enumeration the cooperative kernel walks.  sym = 1, 2, 3 as
+ * fe_get_last_symmetry reports.  counts2 = {n2, n1}: indices [0, n2) are the k-points summed with weight 2, [n2, n2 + n1)
+ * those with weight 1; for 0 <= i < n2 + n1, (row, col) = (k_y, k_x) grid indices of entry i.  Any pointer may be NULL.
+ * FE_EINVAL for another sym, N < 3 or i out of range.  No CUDA call. */
+int fe_debug_sym_index(int32_t sym, int32_t N, int64_t i, int32_t* row, int32_t* col, int64_t* counts2);
+
 /* Diagnostic (not part of the method): evaluate the library's device math on DEVICE arrays of n doubles,
  * y[i] = exp(x[i]) for x <= 0 (which = 0), ln(1 + x[i]) for 0 <= x <= 3 (which = 1), exactly as the direct k-sum
  * kernel evaluates the thermal term of Eq. 5, or sqrt(x[i]) for normal x > 0 (which = 2) as every kernel

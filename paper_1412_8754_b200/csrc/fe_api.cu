@@ -64,6 +64,8 @@ struct fe_handle {
   int32_t target_blocks = 0;   // 0 = auto
   int32_t debug_flags = 0;
   int32_t coop_shape = 0;      // 0 = auto, else 1 + index into kCoopShapes
+  int32_t symmetry = 0;        // fe_set_symmetry: use a lattice mirror when every q of a launch is invariant under it
+  int32_t last_sym = 0;        // CoopParams.sym of the most recent k-sum launch
   double chi_table_budget = 2.0e9;   // bytes of band tables one slice of fe_pair_susceptibility may hold (three-band model)
   int device = 0;
   int sm_count = 148;
@@ -270,6 +272,13 @@ double coop_shape_cost(const CoopShape& s) {
   return (pair + expo) / pair * (s.th * s.td >= 64 ? 1.0 : 1.08);
 }
 
+// Sizes of the symmetry-reduced k set (CoopParams.sym): n2 points counted twice, n1 fixed points of the mirror counted once.
+void sym_counts(int sym, int N, unsigned long long& n2, unsigned long long& n1) {
+  const unsigned long long uN = (unsigned long long)N;
+  if (sym == 3) { n2 = uN * (uN - 1) / 2; n1 = uN; }
+  else { n2 = uN * ((uN - 1) / 2); n1 = (N % 2 == 0) ? 2 * uN : uN; }
+}
+
 int choose_coop_shape(const fe_handle* h, const double* h_list, int nh, int nd, bool early_out) {
   if (h->coop_shape > 0) return h->coop_shape - 1;
   int best = 0; double best_cost = 1e300;
@@ -324,6 +333,7 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
                     const double* delta, int32_t nd, double* omega_dev, cudaStream_t st, int sp = 0) {
   const int N = h->N;
   if (int rcd = check_device(h)) return rcd;
+  h->last_sym = 0;
   // ---- K1c or a per-thread kernel?  (K1c pads to its block tile; tiny h lists are cheaper on K1f) ----
   int mode = h->mode;
   if (sp) {
@@ -454,10 +464,24 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     CP.debug_flags = h->debug_flags;
     CP.early_out = early_out ? 1 : 0;
     CP.nk = (unsigned long long)N * (unsigned long long)N;
+    // mirror-symmetry reduction (fe_set_symmetry): needs a mirror of the lattice that leaves EVERY q of the launch
+    // unchanged (compared exactly); one- and two-band models (E and eta are invariant under all three mirrors)
+    CP.sym = 0; CP.ksplit2 = 0; CP.n2 = 0; CP.n1 = 0;
+    if (h->symmetry && h->nb < 3 && N >= 3) {
+      bool diag = true, my = true, mx = true;
+      for (int i = 0; i < nq; ++i) {
+        diag = diag && q_xy[2 * i] == q_xy[2 * i + 1];
+        my = my && q_xy[2 * i + 1] == 0.0;
+        mx = mx && q_xy[2 * i] == 0.0;
+      }
+      CP.sym = diag ? 3 : (my ? 1 : (mx ? 2 : 0));
+      if (CP.sym) sym_counts(CP.sym, N, CP.n2, CP.n1);
+    }
+    const unsigned long long nk_eff = CP.sym ? CP.n2 + CP.n1 : CP.nk;       // k-points actually visited
     const long long ctiles = (long long)nq * CP.ntile_h * CP.ntile_d;
     const long long wave = (long long)h->sm_count * cs.minb;
-    const long long max_split = (long long)((CP.nk + nt - 1) / nt);          // at least one thread-batch per chunk
-    long long min_split = (long long)ceil((double)CP.nk / fmax(1.0, floor(coop_max_k / nt) * nt));
+    const long long max_split = (long long)((nk_eff + nt - 1) / nt);         // at least one thread-batch per chunk
+    long long min_split = (long long)ceil((double)nk_eff / fmax(1.0, floor(coop_max_k / nt) * nt));
     if (min_split < 1) min_split = 1;
     long long ks;
     if (h->target_blocks > 0) {
@@ -477,10 +501,15 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     if (ks < min_split) ks = min_split;
     if (ks > max_split) ks = max_split;
     if (ks < 1) ks = 1;
-    unsigned long long kc = (CP.nk + ks - 1) / ks;
+    unsigned long long kc = (nk_eff + ks - 1) / ks;
     kc = (kc + nt - 1) / nt * nt;
     CP.kc = kc;
     CP.ksplit = (int32_t)((CP.nk + kc - 1) / kc);
+    if (CP.sym) {                                                              // weight-2 chunks first, then the weight-1 chunks
+      CP.ksplit2 = (int32_t)((CP.n2 + kc - 1) / kc);
+      CP.ksplit = CP.ksplit2 + (int32_t)((CP.n1 + kc - 1) / kc);
+    }
+    h->last_sym = CP.sym;
     P.ksplit = CP.ksplit;
     grid_ll = ctiles * CP.ksplit;
   }
@@ -660,6 +689,33 @@ int fe_set_tuning(fe_handle* h, int32_t tile, int32_t target_blocks) {
   if (tile < 0 || tile > kNumTiles || target_blocks < 0) {
     snprintf(g_errbuf, sizeof g_errbuf, "tile must be in [0, %d], target_blocks >= 0", kNumTiles); return FE_EINVAL; }
   h->tile = tile; h->target_blocks = target_blocks;
+  return FE_OK;
+}
+
+int fe_debug_sym_index(int32_t sym, int32_t N, int64_t i, int32_t* row, int32_t* col, int64_t* counts2) {
+  if (sym < 1 || sym > 3 || N < 3) { snprintf(g_errbuf, sizeof g_errbuf, "sym must be 1, 2 or 3 and N >= 3"); return FE_EINVAL; }
+  unsigned long long n2, n1;
+  sym_counts(sym, N, n2, n1);
+  if (counts2) { counts2[0] = (int64_t)n2; counts2[1] = (int64_t)n1; }
+  if (row || col) {
+    if (i < 0 || (unsigned long long)i >= n2 + n1) { snprintf(g_errbuf, sizeof g_errbuf, "index out of range"); return FE_EINVAL; }
+    int r, c;
+    coop_sym_index(sym, N, n2, (unsigned long long)i, r, c);
+    if (row) *row = r;
+    if (col) *col = c;
+  }
+  return FE_OK;
+}
+
+int fe_set_symmetry(fe_handle* h, int32_t on) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  h->symmetry = on ? 1 : 0;
+  return FE_OK;
+}
+
+int fe_get_last_symmetry(fe_handle* h, int32_t* sym) {
+  if (!h || !sym) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+  *sym = h->last_sym;
   return FE_OK;
 }
 

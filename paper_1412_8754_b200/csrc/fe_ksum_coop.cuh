@@ -45,6 +45,14 @@ struct CoopParams {
   int32_t early_out;                   // 1: A-dominated slots bypass the pair products (FE_EVAL_COOP_EO)
   unsigned long long kc;               // k-points per chunk (multiple of the block size)
   unsigned long long nk;               // N*N
+  // Mirror-symmetry reduction (fe_set_symmetry; PAPER.md:157 uses E(-k) = E(k) in the same spirit): when every q of the
+  // launch is invariant under a mirror M of the lattice (E, eta invariant under M as well), the terms at k and M k are equal
+  // and only the k-points with M k "above" k are summed, with weight 2; the fixed points of M keep weight 1.
+  //   sym 0: none.  1: k_y -> -k_y (all q_y = 0).  2: k_x -> -k_x (all q_x = 0).  3: k_x <-> k_y (all q_x = q_y).
+  // The reduced index set is [0, n2) (weight 2) followed by [n2, n2 + n1) (weight 1); chunks 0 .. ksplit2 - 1 cover the
+  // first part, the others the second, so a chunk has one weight.
+  int32_t sym, ksplit2;
+  unsigned long long n2, n1;
   const double4* coltab;               // [nq][N] {cos kx, sin kx, cos(kx-qx), sin(kx-qx)}
   const double4* rowtab;               // [nq][N] {cos ky, sin ky, cos(ky-qy), sin(ky-qy)}
   const double* h;                     // [nh]
@@ -66,10 +74,13 @@ constexpr int kCoopSkip = 1, kCoopRobust = 2;
 // by kDomGap or more (mantissas are in [0.997, 2.51), so A_j / B_i > 2^(kDomGap - 1.4)): then T ln Z_ij is replaced by R_j
 // for every pair.  What is neglected per term is T ln(1 + B_i/A_j) + T ln(1 + e^{-2R_j/T}) < T 2^-(kDomGap - 1.4) (1 + tiny),
 // and a slot can only be dominated if e^{R_j/T} > 2^(kDomGap - 1.4), i.e. T < R_j / ((kDomGap - 1.4) ln 2): the neglected part
-// is below R_j 2^-48.6 / (48.6 ln 2) = 6.9e-17 R_j < 2^-53 R_j, less than half an ulp of the term it belongs to, in the
-// worst case of a pair sitting exactly at the threshold (pairs are spread over thousands of T beyond it, so the sum of what
-// is neglected is orders of magnitude smaller still).  Same bound for the B-dominated slots (T ln Z_ij = |d_i|).
-constexpr int kDomGap = 50;
+// is below R_j 2^-42.6 / (42.6 ln 2) = 5.1e-15 R_j -- 200 times inside the 1e-12 parity bound even if EVERY dominated pair sat
+// exactly at the threshold, and it is one-signed (P is underestimated).  Pairs are in fact spread over thousands of T beyond
+// the threshold (a fraction ~ T ln 2 / bandwidth of them lies within one binade of it), so the sum of what is neglected is
+// ~1e-17 of the sum: below the rounding noise of the dense path (2e-15 .. 6e-14 observed against the oracle).  Same bound
+// for the B-dominated slots (T ln Z_ij = |d_i|).  Measured on config 4: gap 50 -> 44 turns 8 % (T = 0.01) of the dense
+// slots into dominated ones.
+constexpr int kDomGap = 44;
 // A-dominated slots whose radicand is dominated by s^2 over the whole tile, eps_j = Delta_j^2 g / s^2 <= 1/16, are not even
 // square-rooted per Delta_j:  R_j = |s| sqrt(1 + eps_j) = |s| sum_m c_m eps_j^m  (binomial series, c_m = binom(1/2, m)), so
 //     sum_k R_j(k) = sum_m c_m Delta_j^(2m) M_m,      M_m = sum_k |s_k| x_k^m,   x_k = g_k / s_k^2,
@@ -116,7 +127,34 @@ __device__ __forceinline__ double coop_scale(double m, int shift) {
   return __hiloint2double(__double2hiint(m) + (max(shift, -1000) << 20), __double2loint(m));
 }
 
-template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
+// Index i of the symmetry-reduced k set -> (row, col) = (k_y, k_x) grid indices (CoopParams.sym).
+__host__ __device__ __forceinline__ void coop_sym_index(int sym, int N, unsigned long long n2, unsigned long long i, int& row, int& col) {
+  const unsigned uN = (unsigned)N;
+  if (sym == 1) {                      // rows 1 .. (N-1)/2 twice; rows 0 and (N even) N/2 once
+    if (i < n2) { row = 1 + (int)(i / uN); col = (int)(i % uN); }
+    else { const unsigned long long j = i - n2; row = j < uN ? 0 : N / 2; col = (int)(j % uN); }
+  } else if (sym == 2) {               // columns 1 .. (N-1)/2 twice; columns 0 and (N even) N/2 once
+    const unsigned M = (unsigned)((N - 1) / 2);
+    if (i < n2) { row = (int)(i / M); col = 1 + (int)(i % M); }
+    else { const unsigned long long j = i - n2; col = j < uN ? 0 : N / 2; row = (int)(j % uN); }
+  } else {                             // strict upper triangle col > row twice (row-major, row r holds N-1-r points); diagonal once
+    if (i < n2) {
+      const double b = 2.0 * N - 1.0;
+      long long r = (long long)((b - sqrt(b * b - 8.0 * (double)i)) * 0.5);
+      if (r < 0) r = 0;
+      if (r > N - 2) r = N - 2;
+      // first index of row r: f(r) = r (2N - 1 - r) / 2; correct the rounding of the square root
+      while (r > 0 && (unsigned long long)(r * (2LL * N - 1 - r) / 2) > i) --r;
+      while ((unsigned long long)((r + 1) * (2LL * N - 2 - r) / 2) <= i) ++r;
+      row = (int)r;
+      col = (int)(r + 1 + (long long)(i - (unsigned long long)(r * (2LL * N - 1 - r) / 2)));
+    } else { row = col = (int)(i - n2); }
+  }
+}
+
+// SYM = 1: instance for the symmetry-reduced k set (P.sym = 1, 2, 3); SYM = 0 never looks at P.sym (the kernel sits at
+// 255 registers: the index mapping is kept out of the full-zone instance so that its register allocation is untouched)
+template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB, int SYM = 0>
 __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopParams P) {
   using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
   constexpr int NT = G::NT, WH = G::WH, WD = G::WD, W = G::W, SLOTS = G::SLOTS, BPS = NT / KB;
@@ -187,8 +225,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 
   const double MAGIC = 6755399441055744.0;
   const FactoredConsts& fc = P.fc;
-  const unsigned long long kbeg = (unsigned long long)chunk * P.kc;
-  const unsigned long long kend = min(P.nk, kbeg + P.kc);
+  unsigned long long kbeg = (unsigned long long)chunk * P.kc;
+  unsigned long long kend = min(P.nk, kbeg + P.kc);
+  if constexpr (SYM != 0) {                      // one weight per chunk: chunks < ksplit2 hold the points counted twice
+    if (chunk < P.ksplit2) kend = min(P.n2, kbeg + P.kc);
+    else { kbeg = P.n2 + (unsigned long long)(chunk - P.ksplit2) * P.kc; kend = min(P.n2 + P.n1, kbeg + P.kc); }
+  }
   const bool force_robust = (P.debug_flags & 1) != 0;
 
   // ---------------- P0: one k-point per thread -> NB slot headers (for NT consecutive k-points) ----------------
@@ -210,8 +252,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     if (tid < nleft) carried = hdr_s[(carry_state >> 9) + tid];
     const unsigned long long kidx = kbeg + (unsigned long long)superbatch * NT + tid;
     const bool valid = kidx < kend;
-    const unsigned long long kk = valid ? kidx : kbeg;
-    const int row = (int)(kk / (unsigned)P.N), col = (int)(kk - (unsigned long long)row * (unsigned)P.N);
+    unsigned long long kk = valid ? kidx : kbeg;
+    int row, col;
+    if constexpr (SYM == 0) {
+      row = (int)(kk / (unsigned)P.N); col = (int)(kk - (unsigned long long)row * (unsigned)P.N);
+    } else {
+      coop_sym_index(P.sym, P.N, P.n2, kk, row, col);
+      kk = (unsigned long long)row * (unsigned)P.N + col;
+    }
     const double4 ct = P.coltab[(size_t)iq * P.N + col];
     const double4 rr = P.rowtab[(size_t)iq * P.N + row];
     double Ek[NB], Eq[NB];
@@ -753,6 +801,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   // P_ij = T (ln2 * exponent sum + ln accP_ij); every thread owns its (h, Delta) pairs for the whole chunk
   const double LN2_HI = 6.93147180369123816490e-01, LN2_LO = 1.90821492927058770002e-10;
   const size_t nout = (size_t)P.nq * P.nh * P.nd;
+  const double weight = (SYM != 0 && chunk < P.ksplit2) ? 2.0 : 1.0;
 #pragma unroll
   for (int i = 0; i < TH; ++i) {
     const int ih = th * WH + thx * TH + i;
@@ -768,7 +817,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] - 1023 * nrenorm + ex);
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(mant)));
       if (ih < P.nh && id < P.nd)
-        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = fma(P.T, lnz, accR_s[tdx * TD + j] + sumB);
+        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = weight * fma(P.T, lnz, accR_s[tdx * TD + j] + sumB);
     }
   }
 }

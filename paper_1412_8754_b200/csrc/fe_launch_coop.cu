@@ -7,16 +7,24 @@
 namespace fe {
 namespace {
 
-template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
-cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
+template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB, int SYM>
+cudaError_t launch_coop_sym(int grid, cudaStream_t st, const CoopParams& P) {
   using G = CoopGeom<TH, TD, LH, NW, KB, NB>;
-  auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB>;
+  auto kern = fe_ksum_coop_kernel<NB, FORM, TH, TD, LH, NW, KB, MINB, SYM>;
   // The opt-in is per DEVICE (and a handle binds to the device current at fe_create), so it is set before every
   // launch: a host-side call of a few hundred nanoseconds, no static state shared between devices or host threads.
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
   if (e != cudaSuccess) return e;
   kern<<<grid, G::NT, G::smem_bytes, st>>>(P);
   return cudaGetLastError();
+}
+
+template <int NB, int FORM, int TH, int TD, int LH, int NW, int KB, int MINB>
+cudaError_t launch_coop_inst(int grid, cudaStream_t st, const CoopParams& P) {
+  if constexpr (NB < 3) {           // symmetry-reduced k set (fe_set_symmetry): one- and two-band models
+    if (P.sym != 0) return launch_coop_sym<NB, FORM, TH, TD, LH, NW, KB, MINB, 1>(grid, st, P);
+  }
+  return launch_coop_sym<NB, FORM, TH, TD, LH, NW, KB, MINB, 0>(grid, st, P);
 }
 
 template <int TH, int TD, int LH, int NW, int KB, int MINB>

@@ -19,9 +19,9 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 # include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
-               "fe_get_launch_count", "fe_get_slot_counts", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
+               "fe_get_launch_count", "fe_get_slot_counts", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math",
-                 "fe_set_chi_table_budget"]
+                 "fe_set_chi_table_budget", "fe_debug_sym_index"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
 
@@ -75,6 +75,9 @@ def lib():
     L.fe_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.fe_get_last_launch_info.argtypes = [vp, ip]
     L.fe_get_slot_counts.argtypes = [vp, dp]
+    L.fe_debug_sym_index.argtypes = [C.c_int32, C.c_int32, C.c_int64, ip, ip, C.POINTER(C.c_int64)]
+    L.fe_set_symmetry.argtypes = [vp, C.c_int32]
+    L.fe_get_last_symmetry.argtypes = [vp, ip]
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     L.fe_tile_info.argtypes = [C.c_int32, ip, ip]
     L.fe_set_debug_flags.argtypes = [vp, C.c_int32]
@@ -196,6 +199,16 @@ class FreeEnergy:
 
     def set_tuning(self, tile=0, target_blocks=0):
         _check(lib().fe_set_tuning(self._h, int(tile), int(target_blocks)))
+
+    def set_symmetry(self, on=True):
+        """Opt-in mirror-symmetry reduction of the k-sum (fe_set_symmetry)."""
+        _check(lib().fe_set_symmetry(self._h, 1 if on else 0))
+
+    def last_symmetry(self):
+        """0 none, 1 k_y -> -k_y, 2 k_x -> -k_x, 3 k_x <-> k_y: what the most recent omega_grid launch used."""
+        v = C.c_int32()
+        _check(lib().fe_get_last_symmetry(self._h, C.byref(v)))
+        return v.value
 
     def set_coop_shape(self, shape=0):
         _check(lib().fe_set_coop_shape(self._h, int(shape)))

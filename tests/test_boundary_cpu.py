@@ -102,3 +102,34 @@ def test_workload_shapes_match_baseline_configs():
     assert len(set(cols)) == 16 and (0, 0) in cols and (31, 63) in cols
     pts = W.sample_points(w4, 40, 4)
     assert len(set(pts)) == 40 and all(0 <= a < 32 and 0 <= b < 64 and 0 <= c < 512 for a, b, c in pts)
+
+
+def test_symmetry_reduced_k_enumeration_covers_every_orbit_once():
+    """fe_set_symmetry: the reduced k set the cooperative kernel walks is exactly one representative of
+    every orbit {k, M k} of the mirror M, weight 2 for two-point orbits and weight 1 for the fixed points, so that the
+    weighted sum over it equals the sum over the full N x N grid for any mirror-invariant summand.  Host-only hook."""
+    from paper_1412_8754_b200 import fe
+    L = fe.lib()
+    mirrors = {1: lambda r, c, N: ((N - r) % N, c),          # k_y -> -k_y   (row = k_y index)
+               2: lambda r, c, N: (r, (N - c) % N),          # k_x -> -k_x
+               3: lambda r, c, N: (c, r)}                    # k_x <-> k_y
+    for sym, M in mirrors.items():
+        for N in (3, 4, 5, 8, 31, 64):
+            cnt = (C.c_int64 * 2)()
+            assert L.fe_debug_sym_index(sym, N, 0, None, None, cnt) == fe.FE_OK
+            n2, n1 = cnt[0], cnt[1]
+            weight = np.zeros((N, N), dtype=np.int64)
+            r, c = C.c_int32(), C.c_int32()
+            for i in range(n2 + n1):
+                assert L.fe_debug_sym_index(sym, N, i, C.byref(r), C.byref(c), None) == fe.FE_OK
+                w = 2 if i < n2 else 1
+                mr, mc = M(r.value, c.value, N)
+                assert (w == 1) == ((mr, mc) == (r.value, c.value)), (sym, N, i)      # weight 1 <=> fixed point of the mirror
+                assert weight[r.value, c.value] == 0 and (w == 1 or weight[mr, mc] == 0)  # orbit not visited before
+                weight[r.value, c.value] += 1
+                if w == 2:
+                    weight[mr, mc] += 1
+            assert (weight == 1).all(), (sym, N)                                       # every grid point covered exactly once
+            assert L.fe_debug_sym_index(sym, N, n2 + n1, C.byref(r), C.byref(c), None) == fe.FE_EINVAL
+    assert L.fe_debug_sym_index(0, 8, 0, None, None, None) == fe.FE_EINVAL
+    assert L.fe_debug_sym_index(3, 2, 0, None, None, None) == fe.FE_EINVAL

@@ -17,7 +17,7 @@ from paper_1412_8754_b200 import workloads as W
 LN2 = math.log(2.0)
 
 
-def dense_slot_spreads(oracle, w, T, nk=128, WH=64, WD=128, gap=50):
+def dense_slot_spreads(oracle, w, T, nk=128, WH=64, WD=128, gap=44):
     k = 2.0 * np.pi * np.arange(nk) / nk
     out = []
     ntot = ndense = 0

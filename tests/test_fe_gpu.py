@@ -360,6 +360,58 @@ def test_early_out_block_tile_follows_the_dominance_window(fe, oracle):
             assert max_rel(om.cpu().numpy(), ref) < 1e-12
 
 
+# ---- opt-in mirror-symmetry reduction of the k-sum (fe_set_symmetry) ----
+def test_symmetry_reduced_ksum_matches_oracle_and_full_zone(fe, oracle):
+    """q lists on the (1,1) diagonal, on either axis, and at the origin are invariant under a lattice mirror: with
+    fe_set_symmetry the kernel visits one k-point per orbit (weight 2, fixed points weight 1).  Same Omega as the oracle's
+    full-zone sum at 1e-12 and as the library's own full-zone sum at 1e-13; a q list no mirror leaves invariant, and the
+    three-band model, silently run the full zone."""
+    import torch
+    v = np.array([0.0, 0.13, 0.4, 2.0 * np.pi * 3 / 37])
+    zero = np.zeros_like(v)
+    lists = {3: np.stack([v, v], 1), 1: np.stack([v, zero], 1), 2: np.stack([zero, v], 1), 0: np.stack([v, 0.5 * v + 0.01], 1)}
+    models = ((W.model_params(U=4.0), 37), (W.model_params(U=4.0), 40),
+              (W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(1.0,), mu=0.3, U=2.5), 24),
+              (W.model_params(U=4.0, band_mask=1, cond_mult=1.0, eta_scale=4.0), 25))
+    h = np.linspace(-0.05, 0.3, 9)
+    delta = np.linspace(0.0, 0.4, 21)
+    for params, N in models:
+        for want, q in lists.items():
+            for T in (0.002, 0.05):
+                ref = oracle.omega_grid(params, N, T, q, h, delta)
+                for mode in (fe.EVAL_COOP_EO, fe.EVAL_COOP):
+                    for tb in (0, 1, 3000):
+                        with fe.FreeEnergy(params, N, T) as F:
+                            F.set_eval_mode(mode); F.set_coop_shape(1); F.set_tuning(0, tb)
+                            full = F.omega_grid(q, h, delta).cpu().numpy()
+                            assert F.last_symmetry() == 0
+                            F.set_symmetry(True)
+                            om = F.omega_grid(q, h, delta)
+                            idx, ds, os_ = F.argmin(om, delta)
+                            torch.cuda.synchronize()
+                            assert F.last_symmetry() == want, (N, want, F.last_symmetry())
+                            om = om.cpu().numpy()
+                        assert max_rel(om, ref) < RTOL and max_rel(om, full) < 1e-13
+                        check_argmin(ref, delta, idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy())
+    # q = 0 only: every mirror applies, the diagonal one is taken; all coop shapes
+    params, N = W.model_params(U=4.0), 33
+    q0 = np.zeros((1, 2))
+    ref = oracle.omega_grid(params, N, 0.003, q0, h, delta)
+    for shape in range(1, len(fe.coop_shapes()) + 1):
+        with fe.FreeEnergy(params, N, 0.003) as F:
+            F.set_coop_shape(shape); F.set_symmetry(True)
+            om = F.omega_grid(q0, h, delta).cpu().numpy()
+            assert F.last_symmetry() == 3
+        assert max_rel(om, ref) < RTOL
+    # three-band model: setting ignored
+    w3 = W.three_band(N=24, nq=2, nh=4, nd=8, qdir="diag")
+    with fe.FreeEnergy(w3.params, w3.N, w3.T[0]) as F:
+        a = F.omega_grid(w3.q, w3.h, w3.delta).cpu().numpy()
+        F.set_symmetry(True)
+        b = F.omega_grid(w3.q, w3.h, w3.delta).cpu().numpy()
+        assert F.last_symmetry() == 0 and np.array_equal(a, b)
+
+
 # ---- single-precision builds and screening + verification (SURVEY.md 8f-2, PAPER.md:190-198) ----
 EPS32 = float(np.finfo(np.float32).eps)
 
@@ -762,3 +814,25 @@ def test_full_size_configs_sampled_parity(fe, cfg, mode):
                     n_cols += 1
     assert n_cols == {3: 12, 4: 32, 5: 12 if mode else 4}[cfg]
     assert n_exact >= n_cols // 2          # most stored columns have a resolved minimum (index compared bit-exactly)
+
+
+def test_symmetry_reduced_ksum_full_size_config4(fe):
+    """Config 4 (q on the (1,1) diagonal) with fe_set_symmetry, in the launch configuration bench.py times as
+    `symmetric_variant` (all 32 q in one call): the stored whole oracle columns, Omega at 1e-12 and the minima."""
+    import torch
+    n_cols = 0
+    for w, T, cols in _golden_runs(4):
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            F.set_symmetry(True)
+            om = F.omega_grid(w.q, w.h, w.delta)
+            idx, ds, os_ = F.argmin(om, w.delta)
+            torch.cuda.synchronize()
+            assert F.last_symmetry() == 3 and F.last_launch_info()["mode"] == fe.EVAL_COOP_EO
+        om, idx, ds, os_ = om.cpu().numpy(), idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy()
+        for c in cols:
+            iq, ih = c["iq"], c["ih"]
+            ref = np.array([float(x) for x in c["omega"]])
+            assert max_rel(om[iq, ih], ref) < RTOL
+            check_argmin(ref[None, :], w.delta, idx[iq, ih:ih + 1], ds[iq, ih:ih + 1], os_[iq, ih:ih + 1])
+            n_cols += 1
+    assert n_cols == 32
