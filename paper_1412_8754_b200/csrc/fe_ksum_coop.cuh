@@ -77,7 +77,7 @@ constexpr int kCoopSkip = 1, kCoopRobust = 2;
 // is below R_j 2^-42.6 / (42.6 ln 2) = 5.1e-15 R_j -- 200 times inside the 1e-12 parity bound even if EVERY dominated pair sat
 // exactly at the threshold, and it is one-signed (P is underestimated).  Pairs are in fact spread over thousands of T beyond
 // the threshold (a fraction ~ T ln 2 / bandwidth of them lies within one binade of it), so the sum of what is neglected is
-// ~1e-17 of the sum: below the rounding noise of the dense path (2e-15 .. 6e-14 observed against the oracle).  Same bound
+// ~1e-17 of the sum: below the rounding noise of the dense path (2e-15 .. 6e-14 observed in the parity tests).  Same bound
 // for the B-dominated slots (T ln Z_ij = |d_i|).  Measured on config 4: gap 50 -> 44 turns 8 % (T = 0.01) of the dense
 // slots into dominated ones.
 constexpr int kDomGap = 44;
