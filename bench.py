@@ -241,7 +241,7 @@ def run_reference(args, w):
 
 
 # ----------------------------------------------------------------------------------------------------
-# N > 1: the rank -> q mapping and the gather of the minima (driven on CPU by tests/test_bench_sharding_gloo.py)
+# N > 1: the rank -> q mapping and the gather of the minima (driven on CPU by tests/test_bench_host_logic.py)
 # ----------------------------------------------------------------------------------------------------
 def rank_q(w_q, rank, world, scaling):
     """q-values of this rank.  strong: the workload's own q list, round-robin (sharding.shard_q).  weak: every rank
