@@ -25,7 +25,7 @@ LIB = os.path.join(HERE, "libfe.so")
 LOG = os.path.join(HERE, "build_ptxas.log")
 
 TILES = [(8, 4), (4, 4), (2, 8), (1, 8), (16, 2), (16, 4)]
-COOP_SHAPES = [(16, 4, 4, 4, 4, 2), (16, 4, 1, 4, 2, 2), (8, 4, 4, 4, 4, 3), (8, 4, 1, 4, 2, 2), (16, 4, 2, 4, 2, 2)]
+COOP_SHAPES = [(16, 4, 4, 4, 4, 2), (16, 4, 1, 4, 2, 2), (8, 4, 4, 4, 4, 3), (8, 4, 1, 4, 2, 2), (16, 4, 2, 4, 2, 2), (16, 4, 4, 4, 2, 2)]
 
 HEADERS = [os.path.join(CSRC, f) for f in ("fe_kernels.cuh", "fe_ksum_coop.cuh",  "fe_bands3.cuh", "fe_chi.cuh", "fe_ksum_sp.cuh", "fe_math.cuh",
                                            "fe_launch.h")] + [os.path.join(ROOT, "include", "fe.h"), os.path.join(ROOT, "include", "fe_debug.h")]

@@ -39,7 +39,9 @@ constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 // KB k-points per shared-memory sub-batch, MINB resident blocks per SM.  Block tile = (TH LH) x (TD NW 32/LH).
 struct CoopShape { int th, td, lh, nw, kb, minb; };
 constexpr CoopShape kCoopShapes[] = {{16, 4, 4, 4, 4, 2}, {16, 4, 1, 4, 2, 2}, {8, 4, 4, 4, 4, 3}, {8, 4, 1, 4, 2, 2},
-                                     {16, 4, 2, 4, 2, 2}};   // last: 32 x 256 block tile (one- and two-band models)
+                                     {16, 4, 2, 4, 2, 2},    // 32 x 256 block tile (one- and two-band models)
+                                     {16, 4, 4, 4, 2, 2}};   // 64 x 128 with a half-size sub-batch: the three-band model (12 slots
+                                                             // per sub-batch would take 123 KB of shared memory: one block per SM)
 constexpr int kNumCoopShapes = sizeof(kCoopShapes) / sizeof(kCoopShapes[0]);
 constexpr int kStageSlots = 4;
 constexpr int kSChunksMax = 128;
@@ -260,7 +262,8 @@ cudaError_t launch_coop(int shape, int nb, int form, int grid, cudaStream_t st, 
     case 1: return launch_coop_shape_1(nb, form, grid, st, P);
     case 2: return launch_coop_shape_2(nb, form, grid, st, P);
     case 3: return launch_coop_shape_3(nb, form, grid, st, P);
-    default: return launch_coop_shape_4(nb, form, grid, st, P);
+    case 4: return launch_coop_shape_4(nb, form, grid, st, P);
+    default: return launch_coop_shape_5(nb, form, grid, st, P);
   }
 }
 
@@ -282,7 +285,7 @@ void sym_counts(int sym, int N, unsigned long long& n2, unsigned long long& n1) 
 int choose_coop_shape(const fe_handle* h, const double* h_list, int nh, int nd, bool early_out) {
   if (h->coop_shape > 0) return h->coop_shape - 1;
   int best = 0; double best_cost = 1e300;
-  for (int t = 0; t < kNumCoopShapes; ++t) {
+  for (int t = 0; t < 5; ++t) {                 // (shape 5 is shape 0 with another sub-batch: chosen below, not by cost)
     const CoopShape& s = kCoopShapes[t];
     if (h->nb == 3 && s.lh != 4) continue;
     const int wh = s.th * s.lh, wd = s.td * s.nw * (32 / s.lh);
@@ -295,7 +298,8 @@ int choose_coop_shape(const fe_handle* h, const double* h_list, int nh, int nd, 
   // ~12 % more per dense slot (WD + WH = 288 instead of 192 exponentials per 8192 pairs).  Measured on config 4 (h range
   // 0.3 per 64 values; launches in ms, 64 x 128 vs 32 x 256): T = 0.0005 63.1 / 46.8, 0.001 58.6 / 47.6, 0.002 56.4 / 52.7,
   // 0.004 63.7 / 62.7, 0.006 70.4 / 72.3, 0.01 83.6 / 88.6, 0.02 117.6 / 128.9: the narrow tile wins below window / range ~ 0.5.
-  if (early_out && best == 0 && h->nb < 3 && nh > 32) {
+  if (h->nb == 3 && best == 0) best = 5;        // two resident blocks per SM (measured: dense 625 -> see DESIGN.md section 11 f-1)
+  if (early_out && best == 0 && h->nb < 3 && nh > 32 && (nd + 255) / 256 * 2 <= (nd + 127) / 128) {   // (no extra Delta padding)
     double range = 0.0;
     for (int t0 = 0; t0 < nh; t0 += 64) {
       double lo = h_list[t0], hi = h_list[t0];
