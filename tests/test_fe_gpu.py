@@ -603,6 +603,9 @@ def test_factored_extreme_spreads(fe, oracle):
         parity(fe, oracle, w, T, mode=fe.EVAL_FACTORED)
         for shape in (1, 2):      # the block tile spans the whole wide h list: robust slots chosen on their own
             parity(fe, oracle, w, T, mode=fe.EVAL_COOP, shape=shape)
+            # early-out: robust, fast and dominated slots mixed in one chunk, remainders carried from group to group
+            parity(fe, oracle, w, T, mode=fe.EVAL_COOP_EO, shape=shape, target_blocks=1)
+            parity(fe, oracle, w, T, mode=fe.EVAL_COOP_EO, shape=shape)
 
 
 def test_ksplit_variants_agree_and_match(fe, oracle):
@@ -816,18 +819,20 @@ def test_full_size_configs_sampled_parity(fe, cfg, mode):
     assert n_exact >= n_cols // 2          # most stored columns have a resolved minimum (index compared bit-exactly)
 
 
-def test_symmetry_reduced_ksum_full_size_config4(fe):
-    """Config 4 (q on the (1,1) diagonal) with fe_set_symmetry, in the launch configuration bench.py times as
-    `symmetric_variant` (all 32 q in one call): the stored whole oracle columns, Omega at 1e-12 and the minima."""
+@pytest.mark.parametrize("cfg,sym,ncols", [(4, 3, 32), (3, 1, 12), (5, 1, 12)])
+def test_symmetry_reduced_ksum_full_size_configs(fe, cfg, sym, ncols):
+    """Configs 3-5 with fe_set_symmetry (config 4: q on the (1,1) diagonal, k_x <-> k_y, the launch configuration bench.py
+    times as `symmetric_variant`; configs 3 and 5: q = (q_x, 0), k_y -> -k_y), all q in one call: the stored whole oracle
+    columns, Omega at 1e-12 and the minima."""
     import torch
     n_cols = 0
-    for w, T, cols in _golden_runs(4):
+    for w, T, cols in _golden_runs(cfg):
         with fe.FreeEnergy(w.params, w.N, T) as F:
             F.set_symmetry(True)
             om = F.omega_grid(w.q, w.h, w.delta)
             idx, ds, os_ = F.argmin(om, w.delta)
             torch.cuda.synchronize()
-            assert F.last_symmetry() == 3 and F.last_launch_info()["mode"] == fe.EVAL_COOP_EO
+            assert F.last_symmetry() == sym and F.last_launch_info()["mode"] == fe.EVAL_COOP_EO
         om, idx, ds, os_ = om.cpu().numpy(), idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy()
         for c in cols:
             iq, ih = c["iq"], c["ih"]
@@ -835,4 +840,4 @@ def test_symmetry_reduced_ksum_full_size_config4(fe):
             assert max_rel(om[iq, ih], ref) < RTOL
             check_argmin(ref[None, :], w.delta, idx[iq, ih:ih + 1], ds[iq, ih:ih + 1], os_[iq, ih:ih + 1])
             n_cols += 1
-    assert n_cols == 32
+    assert n_cols == ncols
