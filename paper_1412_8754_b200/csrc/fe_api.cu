@@ -356,8 +356,19 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     if (h->coop_shape == 0 && h->nb < 3) {
       const CoopShape& cs = kCoopShapes[cshape];
       const int wh = cs.th * cs.lh, wd = cs.td * cs.nw * (32 / cs.lh);
-      const double coop_cost = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd) *
-                               coop_shape_cost(cs) * kCoopVsFactored;
+      double coop_cost = (double)((nh + wh - 1) / wh * wh) * (double)((nd + wd - 1) / wd * wd) *
+                         coop_shape_cost(cs) * kCoopVsFactored;
+      if (early_out) {
+        // Early-out leaves only the slots within the dominance window of the Fermi surface for the pair products: of the
+        // dense cost roughly 0.1 (classification, dominated sums) + (h range + 2 windows) / band half-width remains
+        // (config 4: 0.13 at T = 0.001, 0.18 at T = 0.01; measured 0.13 / 0.22).  At low T that makes K1c the cheaper
+        // kernel even on grids far smaller than its block tile (the paper's benchmark shape, 1 h x 200 Delta at N = 2000:
+        // 3.8 ms per-thread kernel, 2.7 ms K1c with the 8 x 512 tile).
+        double hlo = h_list[0], hhi = h_list[0];
+        for (int i = 1; i < nh; ++i) { hlo = fmin(hlo, h_list[i]); hhi = fmax(hhi, h_list[i]); }
+        const double window = (double)kDomGap * h->T * 0.6931471805599453;
+        coop_cost *= fmin(1.0, 0.1 + (hhi - hlo + 2.0 * window) / band_half_width(h->p));
+      }
       const int lt = choose_tile_mode(0, FE_EVAL_FACTORED, nh, nd);
       const double legacy_cost = (double)((nh + kTiles[lt].th - 1) / kTiles[lt].th * kTiles[lt].th) *
                                  (double)((nd + kTiles[lt].td - 1) / kTiles[lt].td * kTiles[lt].td) * kTileCostFactored[lt];
