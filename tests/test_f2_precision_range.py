@@ -62,3 +62,20 @@ def test_pair_sums_of_dense_slots_exceed_the_binary32_range(oracle):
     assert sp_warm.max() < 60
     # binary64 as used by the kernels: every one of these slots is a "fast" slot (spread <= kSpread = 900)
     assert sp_cold.max() < 900
+
+
+def test_dense_share_by_block_tile_and_per_pair(oracle):
+    """The figures DESIGN.md section 5 quotes for the early-out classification of config 4 (dominance gap 2^50, as measured
+    when the 32 x 256 tile was introduced): share of (k, band) slots that stay dense per 64 x 128 tile, per 32 x 256 tile and
+    per single (h, Delta) pair.  A narrower tile along h leaves fewer slots dense at low T; at T = 0.01 the window is as
+    wide as the h range and the tile hardly matters.  (The per-pair case is evaluated on every 8th h and 32nd Delta.)"""
+    w = W.config(4)
+    got = {}
+    for T in (0.001, 0.01):
+        for WH, WD in ((64, 128), (32, 256)):
+            got[T, WH, WD] = dense_slot_spreads(oracle, w, T, nk=96, WH=WH, WD=WD, gap=50)[1]
+        sub = W.Workload("cfg4_sub", w.params, w.N, w.T, w.q, w.h[::8].copy(), w.delta[::32].copy())
+        got[T, 1, 1] = dense_slot_spreads(oracle, sub, T, nk=96, WH=1, WD=1, gap=50)[1]
+    assert 0.105 < got[0.001, 64, 128] < 0.13 and 0.075 < got[0.001, 32, 256] < 0.10 and 0.015 < got[0.001, 1, 1] < 0.03
+    assert 0.20 < got[0.01, 64, 128] < 0.23 and 0.18 < got[0.01, 32, 256] < 0.21 and 0.15 < got[0.01, 1, 1] < 0.19
+    assert got[0.001, 32, 256] < 0.8 * got[0.001, 64, 128] and got[0.01, 32, 256] > 0.88 * got[0.01, 64, 128]
