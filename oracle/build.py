@@ -14,8 +14,18 @@ LIB = os.path.join(HERE, "libfe_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    fresh = lambda: os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC)     # noqa: E731
+    if not force and fresh():
         return LIB
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:       # one builder at a time (parallel test workers, ranks)
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and fresh():
+            return LIB
+        return _build_locked()
+
+
+def _build_locked() -> str:
     cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC",
            "-shared", "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC, "-lm"]
     subprocess.run(cmd, check=True)

@@ -77,6 +77,16 @@ def stale() -> bool:
 def build(force: bool = False, extra=(), verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
+    # one builder at a time: several ranks of a multi-GPU launch may find the library stale at once
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not stale():
+            return LIB                       # another process built it while this one waited
+        return _build_locked(extra, verbose)
+
+
+def _build_locked(extra, verbose) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ, exist_ok=True)
 
