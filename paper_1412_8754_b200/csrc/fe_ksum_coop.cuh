@@ -112,9 +112,14 @@ struct CoopGeom {
   static constexpr int DPAD = 16;              // room behind the A-dominated list: its neutral padding (< 8) + one prefetch round (8)
   static constexpr int HTOT = NT * NB + 2 * SLOTS + DPAD;   // header array: dense slots compacted at the front (behind the < SLOTS
                                                // slots carried over from the previous group), B- then A-dominated slots at the back
+  // Shapes with all 32 lanes of a warp along Delta (LH = 1: WD = 512) have wide slot rows; with the moment arrays they would
+  // take 118 KB of shared memory, one block per SM (measured on config 5: the FP64 pipe below 40 %).  For them the Delta^2
+  // list of the tile and the 2^(j/256) table are read from global memory (4 + 2 KB, L1-resident) instead of a shared copy.
+  static constexpr bool SLIM = LH == 1;
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
-      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * (256 + WD + WH + 8 + WD + NT + kMomN * NT + kMomN * NW) + sizeof(int) * 2 * (NW + 2);
+      sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * ((SLIM ? 0 : 256 + WD) + WH + 8 + WD + NT + kMomN * NT + kMomN * NW) +
+      sizeof(int) * 2 * (NW + 2);
   // position of A_j (j = index in the block tile's Delta list) in a slot row: the two doubles a thread reads with
   // one LDS.128 are adjacent and consecutive threads follow each other, so a warp's load is one 128-byte wavefront
   __host__ __device__ static constexpr int posA(int jg) { return ((jg % TD) / 2) * SA + (jg / TD) * 2 + (jg & 1); }
@@ -165,9 +170,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   extern __shared__ __align__(16) unsigned char smem_raw[];
   CoopHdr* const hdr_s = reinterpret_cast<CoopHdr*>(smem_raw);                       // [HTOT]
   double* const buf_s = reinterpret_cast<double*>(hdr_s + G::HTOT);                  // 2 x {[SLOTS][W] values, [SLOTS] int2}
-  double* const tab256 = buf_s + 2 * G::BUF_DOUBLES;                                 // [256]
-  double* const d2_s = tab256 + 256;                                                 // [WD]
-  double* const h_s = d2_s + WD;                                                     // [WH]
+  double* const tab256_s = buf_s + 2 * G::BUF_DOUBLES;                               // [256]   (not for SLIM shapes)
+  double* const d2_s = tab256_s + 256;                                               // [WD]    (not for SLIM shapes)
+  double* const h_s = G::SLIM ? tab256_s : d2_s + WD;                                // [WH]
+  const double* const tab256 = G::SLIM ? P.tabs->exp2_j256 : tab256_s;
   double* const rng_s = h_s + WH;                                                    // hmin hmax d2min d2max (+pad)
   double* const accR_s = rng_s + 8;                                                  // [WD] sums of R_j over A-dominated slots
   double* const accB_s = accR_s + WD;                                                // [NT / WH][WH] sums of |d_i| over B-dominated slots
@@ -188,8 +194,15 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   const int tdx = warp * G::LD + (lane % G::LD);
   const int thx = lane / G::LD;
 
-  for (int i = tid; i < 256; i += NT) tab256[i] = P.tabs->exp2_j256[i];
-  for (int i = tid; i < WD; i += NT) d2_s[i] = P.d2[min(td * WD + i, P.nd - 1)];
+  // Delta_j^2 of the block tile, j = index in the tile (entries past the end of the list repeat the last one)
+  auto d2at = [&](int i) -> double {
+    if constexpr (G::SLIM) return P.d2[min(td * WD + i, P.nd - 1)];
+    else return d2_s[i];
+  };
+  if constexpr (!G::SLIM) {
+    for (int i = tid; i < 256; i += NT) tab256_s[i] = P.tabs->exp2_j256[i];
+    for (int i = tid; i < WD; i += NT) d2_s[i] = P.d2[min(td * WD + i, P.nd - 1)];
+  }
   for (int i = tid; i < WH; i += NT) h_s[i] = P.h[min(th * WH + i, P.nh - 1)];
   for (int i = tid; i < WD; i += NT) accR_s[i] = 0.0;
   accB_s[tid] = 0.0;
@@ -200,9 +213,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   for (int pq = 0; pq < TH * TD; ++pq) myE[pq * NT] = 0;
   __syncthreads();
   if (warp == 0) {   // ranges of the block tile's lists (any order)
-    double hmn = h_s[0], hmx = h_s[0], dmn = d2_s[0], dmx = d2_s[0];
+    double hmn = h_s[0], hmx = h_s[0], dmn = d2at(0), dmx = dmn;
     for (int i = lane; i < WH; i += 32) { hmn = fmin(hmn, h_s[i]); hmx = fmax(hmx, h_s[i]); }
-    for (int i = lane; i < WD; i += 32) { dmn = fmin(dmn, d2_s[i]); dmx = fmax(dmx, d2_s[i]); }
+    for (int i = lane; i < WD; i += 32) { const double v = d2at(i); dmn = fmin(dmn, v); dmx = fmax(dmx, v); }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       hmn = fmin(hmn, __shfl_xor_sync(0xffffffffu, hmn, o));
@@ -383,7 +396,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const double2* const dm = reinterpret_cast<const double2*>(&hdr_s[DEND - ndom].s2);   // entry i at dm[2 i]: {s2, g2}
 #pragma unroll 1
       for (int r = 0; r < WD / NT; ++r) {
-        const double d2 = d2_s[tid + r * NT];
+        const double d2 = d2at(tid + r * NT);
         constexpr int UD = 8;                                // independent sqrt chains, fixed order
         double acc[UD];
         double2 g[UD];
@@ -442,7 +455,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
 #pragma unroll 1
     for (int r = 0; r < WD / NT; ++r) {
       const int jg = tid + r * NT;
-      const double d2 = d2_s[jg];
+      const double d2 = d2at(jg);
       const int pos = G::posA(jg);
 #pragma unroll 1
       for (int sl0 = 0; sl0 < SLOTS; sl0 += U) {
@@ -553,7 +566,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
   double d2r[RA];
   int posAr[RA];
 #pragma unroll
-  for (int r = 0; r < RA; ++r) { d2r[r] = d2_s[tid + r * NT]; posAr[r] = G::posA(tid + r * NT); }
+  for (int r = 0; r < RA; ++r) { d2r[r] = d2at(tid + r * NT); posAr[r] = G::posA(tid + r * NT); }
   const int ibB = tid % WH, slbB = tid / WH, posBr = G::posB(ibB);
   const double hvB = h_s[ibB];
 
@@ -784,7 +797,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     }
     __syncthreads();
     for (int jg = tid; jg < WD; jg += NT) {
-      const double d2 = d2_s[jg];
+      const double d2 = d2at(jg);
       double poly = 0.0;
 #pragma unroll
       for (int m = kMomN - 1; m >= 0; --m) {
