@@ -34,6 +34,11 @@ int fe_tile_info(int32_t tile, int32_t* th, int32_t* td);   /* FE_EINVAL past th
  * resident blocks per SM}; FE_EINVAL past the end of the table. */
 int fe_set_coop_shape(fe_handle* h, int32_t shape);
 int fe_coop_shape_info(int32_t shape, int32_t* info6);
+/* Resident blocks per SM of one instance of the cooperative kernel on the CURRENT device (occupancy query with the
+ * instance's shared memory and registers): shape from 1 as above, nbands 1..3, form_factor FE_FORM_*, sym 0 / 1 (the
+ * fe_set_symmetry instance).  A test compares it with the launch bound of fe_coop_shape_info, so that an instance that
+ * stops fitting (more shared memory, more registers) is noticed.  FE_EINVAL if the shape has no such instance.       */
+int fe_debug_coop_occupancy(int32_t shape, int32_t nbands, int32_t form_factor, int32_t sym, int32_t* blocks_per_sm);
 /* Test hook for FE_EVAL_FACTORED / FE_EVAL_COOP(_EO): bit 0 = always take the robust per-pair path (this also switches
  * the early-out of FE_EVAL_COOP_EO off), bit 1 = never use the per-tile h recurrence (FACTORED).  Results are the same
  * sums; only the code path changes (lets tests cover each path).                                            */

@@ -742,6 +742,25 @@ int fe_set_coop_shape(fe_handle* h, int32_t shape) {
   return FE_OK;
 }
 
+int fe_debug_coop_occupancy(int32_t shape, int32_t nbands, int32_t form_factor, int32_t sym, int32_t* blocks_per_sm) {
+  if (shape < 1 || shape > kNumCoopShapes || nbands < 1 || nbands > 3 || form_factor < 0 || form_factor > 1 || !blocks_per_sm) {
+    snprintf(g_errbuf, sizeof g_errbuf, "no such instance"); return FE_EINVAL; }
+  int blocks = 0;
+  cudaError_t e;
+  switch (shape - 1) {
+    case 0: e = occupancy_coop_shape_0(nbands, form_factor, sym, &blocks); break;
+    case 1: e = occupancy_coop_shape_1(nbands, form_factor, sym, &blocks); break;
+    case 2: e = occupancy_coop_shape_2(nbands, form_factor, sym, &blocks); break;
+    case 3: e = occupancy_coop_shape_3(nbands, form_factor, sym, &blocks); break;
+    case 4: e = occupancy_coop_shape_4(nbands, form_factor, sym, &blocks); break;
+    default: e = occupancy_coop_shape_5(nbands, form_factor, sym, &blocks); break;
+  }
+  if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); snprintf(g_errbuf, sizeof g_errbuf, "this shape has no instance for %d bands", nbands); return FE_EINVAL; }
+  FE_CUDA(e);
+  *blocks_per_sm = blocks;
+  return FE_OK;
+}
+
 int fe_coop_shape_info(int32_t shape, int32_t* info6) {
   if (shape < 1 || shape > kNumCoopShapes || !info6) { snprintf(g_errbuf, sizeof g_errbuf, "no such shape"); return FE_EINVAL; }
   const CoopShape& s = kCoopShapes[shape - 1];

@@ -115,7 +115,8 @@ struct CoopGeom {
   // Shapes with all 32 lanes of a warp along Delta (LH = 1: WD = 512) have wide slot rows; with the moment arrays they would
   // take 118 KB of shared memory, one block per SM (measured on config 5: the FP64 pipe below 40 %).  For them the Delta^2
   // list of the tile and the 2^(j/256) table are read from global memory (4 + 2 KB, L1-resident) instead of a shared copy.
-  static constexpr bool SLIM = LH == 1;
+  // (Likewise the 8 x 4 register-tile shape, whose launch bound is three blocks per SM: 77 -> 74 KB.)
+  static constexpr bool SLIM = LH == 1 || TH * TD < 64;
   static constexpr size_t smem_bytes =
       sizeof(CoopHdr) * HTOT + 2 * sizeof(double) * (size_t)BUF_DOUBLES + 2 * sizeof(int) * (size_t)SLOTS * W +
       sizeof(int) * (size_t)TH * TD * NT + sizeof(double) * ((SLIM ? 0 : 256 + WD) + WH + 8 + WD + NT + kMomN * NT + kMomN * NW) +

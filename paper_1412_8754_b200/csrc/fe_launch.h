@@ -30,7 +30,8 @@ FE_DECL_TILE(0) FE_DECL_TILE(1) FE_DECL_TILE(2) FE_DECL_TILE(3) FE_DECL_TILE(4) 
 #undef FE_DECL_TILE
 
 // K1c, shape index = position in kCoopShapes of fe_api.cu
-#define FE_DECL_COOP(i) cudaError_t launch_coop_shape_##i(int nb, int form, int grid, cudaStream_t st, const CoopParams& P);
+#define FE_DECL_COOP(i) cudaError_t launch_coop_shape_##i(int nb, int form, int grid, cudaStream_t st, const CoopParams& P); \
+  cudaError_t occupancy_coop_shape_##i(int nb, int form, int sym, int* blocks);
 FE_DECL_COOP(0) FE_DECL_COOP(1) FE_DECL_COOP(2) FE_DECL_COOP(3) FE_DECL_COOP(4) FE_DECL_COOP(5)
 #undef FE_DECL_COOP
 

@@ -21,7 +21,7 @@ EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
                "fe_get_launch_count", "fe_get_slot_counts", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math",
-                 "fe_set_chi_table_budget", "fe_debug_sym_index"]
+                 "fe_set_chi_table_budget", "fe_debug_sym_index", "fe_debug_coop_occupancy"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
 
 
@@ -76,6 +76,7 @@ def lib():
     L.fe_get_last_launch_info.argtypes = [vp, ip]
     L.fe_get_slot_counts.argtypes = [vp, dp]
     L.fe_debug_sym_index.argtypes = [C.c_int32, C.c_int32, C.c_int64, ip, ip, C.POINTER(C.c_int64)]
+    L.fe_debug_coop_occupancy.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, ip]
     L.fe_set_symmetry.argtypes = [vp, C.c_int32]
     L.fe_get_last_symmetry.argtypes = [vp, ip]
     L.fe_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
@@ -158,6 +159,13 @@ def coop_shapes():
         out.append(tuple(a))
         i += 1
     return out
+
+
+def coop_occupancy(shape, nbands=2, form_factor=1, sym=0):
+    """Resident blocks per SM of one cooperative-kernel instance on the current device (fe_debug_coop_occupancy)."""
+    v = C.c_int32()
+    _check(lib().fe_debug_coop_occupancy(int(shape), int(nbands), int(form_factor), int(sym), C.byref(v)))
+    return v.value
 
 
 def fp64_peak_probe(blocks=148 * 16, iters=1 << 16, stream=None):
