@@ -558,6 +558,59 @@ def test_randomised_grids_all_models(fe, oracle):
     assert n_ill < 0.01 * n_total, (n_ill, n_total)
 
 
+def test_randomised_variants_shapes_symmetry_chunkings(fe, oracle):
+    """Seeded random grids through the variants the previous test does not reach: forced block shapes, the early-out and
+    the dense mode, the full zone and fe_set_symmetry (q lists on the diagonal or an axis, or generic: then the setting must
+    be ignored), random k-chunkings.  Same acceptance rule as test_randomised_grids_all_models."""
+    import torch
+    rng = np.random.default_rng(20141232)
+    nshapes = len(fe.coop_shapes())
+    n_ill = n_total = 0
+    for case in range(40):
+        model = int(rng.choice([1, 2, 2, 3]))
+        N = int(rng.integers(5, 80))
+        T = float(10.0 ** rng.uniform(-4.3, 0))
+        nq, nh, nd = int(rng.integers(1, 4)), int(rng.choice([1, 3, 16, 17, 31, 33, 64, 65])), int(rng.choice([1, 7, 127, 129, 255, 257, 300]))
+        if model == 3:
+            p, hs, ds, qs = W.model_params(model=3, mu=W.THREE_BAND_MU + float(rng.uniform(-0.2, 0.2)), U=float(rng.uniform(0.8, 2.0))), 0.08, 0.2, 0.8
+        elif model == 2:
+            p, hs, ds, qs = W.model_params(U=float(rng.uniform(2, 6)), mu=W.TWO_BAND_MU + float(rng.uniform(-1, 1))), 0.4, 0.5, 0.8
+        else:
+            p, hs, ds, qs = W.model_params(model=1, form_factor=int(rng.integers(0, 2)), t=(float(rng.uniform(0.5, 1.5)),),
+                                           mu=float(rng.uniform(-3, 3)), U=float(rng.uniform(1, 5))), 0.5, 0.6, 1.5
+        kind = int(rng.integers(0, 4))                       # q list: generic, diagonal, x axis, y axis
+        v = rng.uniform(-qs, qs, size=nq)
+        q = {0: rng.uniform(-qs, qs, size=(nq, 2)), 1: np.stack([v, v], 1), 2: np.stack([v, 0 * v], 1), 3: np.stack([0 * v, v], 1)}[kind]
+        h = np.sort(rng.uniform(-0.3 * hs, hs, size=nh)) * float(rng.choice([1.0, 1.0, 10.0]))
+        d = np.sort(rng.uniform(-0.2 * ds, ds, size=nd))
+        ref = oracle.omega_grid(p, N, T, q, h, d)
+        mag = None
+        shape = int(rng.integers(0, nshapes + 1))
+        if model == 3 and shape in (2, 4, 5):
+            shape = 0
+        for mode in (fe.EVAL_COOP_EO, fe.EVAL_COOP):
+            for sym in (0, 1):
+                with fe.FreeEnergy(p, N, T) as F:
+                    F.set_eval_mode(mode); F.set_coop_shape(shape); F.set_tuning(0, int(rng.choice([0, 1, 37, 3000]))); F.set_symmetry(bool(sym))
+                    om = F.omega_grid(q, h, d)
+                    idx, _, os_ = F.argmin(om, d)
+                    torch.cuda.synchronize()
+                    used = F.last_symmetry()
+                    coop = F.last_launch_info()["mode"] in (fe.EVAL_COOP, fe.EVAL_COOP_EO)
+                    om = om.cpu().numpy()
+                assert used == ({0: 0, 1: 3, 2: 1, 3: 2}[kind] if (sym and model < 3 and coop and N >= 3) else 0), (case, kind, sym, used)
+                err = np.abs(om - ref)
+                miss = err > RTOL * np.abs(ref)
+                if miss.any():
+                    if mag is None:
+                        mag = oracle.omega_grid_magnitude(p, N, T, q, h, d)
+                    assert np.all(mag[miss] > 100.0 * np.abs(ref[miss])) and np.all(err[miss] <= 1e-14 * mag[miss]), (case, model, N, T, shape, mode, sym)
+                    n_ill += int(miss.sum())
+                n_total += ref.size
+                assert np.array_equal(idx.cpu().numpy(), np.argmin(om, axis=-1).astype(np.int32))
+    assert n_ill < 0.01 * n_total, (n_ill, n_total)
+
+
 def test_full_size_properties_in_bench_launch_configuration(fe):
     """Whole config-3, config-4 and config-5 steps exactly as bench.py launches them (all q, all h, all Delta in one
     call): properties that hold at any size -- Omega(q) = Omega(-q) (O4), the early-out and the dense variant agree, the
