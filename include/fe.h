@@ -194,6 +194,58 @@ int fe_scan_host(fe_handle* h,
                  double* omega_host, int32_t* idx_host, double* delta_star_host, double* omega_star_host,
                  void* cuda_stream);
 
+/* Omega on a SMALL grid without any allocation, for callers that cannot let this library call cudaMalloc.
+ *
+ * Who that is.  Every other entry point works on an fe_handle, and a handle allocates: fe_create makes the math tables,
+ * and fe_omega_grid releases and re-makes the handle's scratch (cudaFree + cudaMalloc, plus pinned staging) whenever a call
+ * needs more than any earlier call did.  That does not suit
+ *   - a process in which something else already owns the device memory -- typically a framework's caching allocator (the
+ *     PyTorch one this library's Python binding sits next to) that has reserved nearly all of HBM: a cudaMalloc from
+ *     outside that pool then fails although the job as a whole has memory to spare;
+ *   - a caller that runs other work on the same GPU at the same time: cudaMalloc and cudaFree make the whole device wait,
+ *     so a scan that grows its grid stalls the other streams at a moment the caller does not choose;
+ *   - a caller whose memory budget is fixed when the job starts (a service with a hard per-process limit) and who
+ *     therefore needs the library's footprint to be a constant known in advance.
+ * For them this function computes the same Omega (Eq. 4 / Eq. 5; steps S1-S9) with all of its working
+ * memory in ONE fixed array compiled into the library (a file-scope __device__ array of FE_STATIC_BYTES_MAX bytes or less,
+ * about 7.8 MiB).  That array is part of the library image: every GPU on which the library's code gets loaded holds it
+ * from then until the process exits, whether or not this function is ever called.  The function takes no handle and calls
+ * no cudaMalloc, cudaFree, cudaMallocHost or other allocating routine; the caller brings the inputs and the output.
+ *
+ *   params, N, T : as fe_create (same validation).  One- and two-band models only; FE_MODEL_THREE_BAND is FE_EINVAL
+ *                  (its per-q band tables do not fit a fixed array of this size).
+ *   q_xy, h_list, delta : HOST lists as fe_omega_grid; copied before the call returns (from pageable memory, so the
+ *                  copy call may first wait for earlier work on cuda_stream).
+ *   omega_dev    : DEVICE, nq*nh*nd doubles, layout as fe_omega_grid; caller-owned.
+ * Limits (fe_static_limits reports them; beyond any of them the call returns FE_EINVAL with a message that names the
+ * quantity, its value and the limit, and touches nothing):
+ *   2 nq + nh + nd <= FE_STATIC_MAX_LIST,  nq N <= FE_STATIC_MAX_TRIG,  nq nh nd <= FE_STATIC_MAX_OUT,
+ *   ceil(N / 256) nq nh nd <= FE_STATIC_MAX_PARTIAL.   Example that fits: N = 1024, 1 q, 16 h, 512 Delta.
+ * It evaluates every term directly (the FE_EVAL_DIRECT formulation of fe_debug.h, the slowest and most literal one), which
+ * is adequate at these sizes; results agree with fe_omega_grid to rounding (~1e-14 relative) and are deterministic.
+ *
+ * First call on a device: it looks up the device address of the array (cudaGetSymbolAddress, once per device, with that
+ * device current) and copies the math tables into it with a host-synchronous cudaMemcpy.  Make that first call during
+ * start-up, before any stream capture begins and before the phase in which the device must not be disturbed.
+ * Later calls only enqueue work on cuda_stream and return without synchronising.
+ *
+ * Sharing: all calls on a device use the SAME array, and it keeps what the last call left in it.  Each call rewrites every
+ * word it later reads (tables, lists, partial sums), so stale contents never reach a result and nothing needs to be zeroed.
+ * But two calls whose GPU work overlaps -- different streams, or different host threads -- overwrite each other's
+ * partial sums and both results are garbage: keep all calls of a device on one stream, or order them with events.
+ * Errors: FE_EINVAL (arguments, limits), FE_EARCH, FE_ECUDA.                                                     */
+#define FE_STATIC_MAX_LIST    4096      /* doubles */
+#define FE_STATIC_MAX_TRIG    32768     /* table entries */
+#define FE_STATIC_MAX_OUT     32768     /* Omega values per call */
+#define FE_STATIC_MAX_PARTIAL 720896    /* doubles: k-chunks x Omega values */
+#define FE_STATIC_BYTES_MAX   (8u << 20)
+int fe_omega_grid_static(const fe_model_params* params, int32_t N, double T,
+                         const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                         const double* delta, int32_t nd, double* omega_dev, void* cuda_stream);
+/* limits5 (HOST) = {FE_STATIC_MAX_LIST, FE_STATIC_MAX_TRIG, FE_STATIC_MAX_OUT, FE_STATIC_MAX_PARTIAL, bytes of the fixed
+ * array as built}.  Host-only, no CUDA call. */
+int fe_static_limits(int64_t* limits5);
+
 /* Kernel timing for roofline reports.  When enabled, fe_omega_grid brackets its k-sum kernel (K1) with
  * CUDA events on the launching stream; after the caller has synchronised the stream, fe_get_timing returns
  * the duration of the most recent K1 launch (ms) and the number of (k, band, q, h, Delta) terms it evaluated. */

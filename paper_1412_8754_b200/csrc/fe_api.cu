@@ -5,6 +5,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include "../../include/fe.h"
@@ -1144,6 +1145,178 @@ const char* fe_strerror(int code) {
     case FE_EINVAL: case FE_ENOMEM: case FE_ECUDA: case FE_EARCH: return g_errbuf;
     default: return "unknown error code";
   }
+}
+
+}  // extern "C"
+
+// =====================================================================================================
+// fe_omega_grid_static: Omega on a small grid for callers that must not allocate (include/fe.h has the contract)
+// =====================================================================================================
+//
+// Everything fe_omega_grid keeps in cudaMalloc'ed handle scratch (the exp / log tables, the device copy of the parameter
+// lists, the trig tables of K0, the constant-term partial sums of KS and the [k-chunk][q, h, Delta] partial sums that K1
+// writes and K2 adds up) lives here in ONE fixed array that is part of the library image: the driver places it when the
+// library's code is loaded onto a device and it stays there, on every device that loads the library, until the process
+// exits.  The kernels are the ones fe_omega_grid uses in FE_EVAL_DIRECT mode (K0, KS, K1 with the 4 x 4 register tile,
+// K2); only where their scratch comes from differs.
+namespace {
+
+constexpr size_t kStTabsBytes = 8192;                    // MathTabs (6.7 KB), padded
+constexpr size_t kStListMax = FE_STATIC_MAX_LIST;        // doubles: q (2 nq) | h (nh) | Delta^2 (nd)
+constexpr size_t kStTrigMax = FE_STATIC_MAX_TRIG;        // entries of each trig table: nq * N
+constexpr size_t kStOutMax = FE_STATIC_MAX_OUT;          // nq * nh * nd
+constexpr size_t kStPartialMax = FE_STATIC_MAX_PARTIAL;  // doubles: k-chunks * nq * nh * nd
+constexpr size_t kStOffList = kStTabsBytes;
+constexpr size_t kStOffCol = kStOffList + kStListMax * sizeof(double);
+constexpr size_t kStOffRow = kStOffCol + kStTrigMax * sizeof(double4);
+constexpr size_t kStOffSpart = kStOffRow + kStTrigMax * sizeof(double4);
+constexpr size_t kStOffPartial = kStOffSpart + kStTrigMax * sizeof(double);     // nq * min(N, 128) <= nq * N
+constexpr size_t kStBytes = kStOffPartial + kStPartialMax * sizeof(double);
+static_assert(sizeof(MathTabs) <= kStTabsBytes, "table block too small");
+static_assert(kStOffList % 256 == 0 && kStOffCol % 256 == 0 && kStOffRow % 256 == 0 && kStOffSpart % 256 == 0 &&
+              kStOffPartial % 256 == 0, "sub-blocks keep the 256-byte alignment of the array");
+static_assert(kStBytes <= (size_t)8 << 20, "the fixed scratch is meant to stay modest (8 MiB)");
+
+}  // namespace
+
+// The scratch itself.  In HOST code the name `fe_static_scratch` is only the runtime's handle for the symbol, NOT a device
+// address: it must go through cudaGetSymbolAddress (static_setup below) before a kernel can be given a pointer into it.
+static __device__ __align__(256) unsigned char fe_static_scratch[kStBytes];
+
+namespace {
+
+constexpr int kStMaxDevices = 64;
+struct StaticDev {
+  bool ready = false;
+  unsigned char* base = nullptr;   // device address of fe_static_scratch on this device
+  int sm_count = 0;
+};
+StaticDev g_static_dev[kStMaxDevices];      // plain static storage: no allocation at first use
+std::mutex g_static_mutex;                  // two host threads making the first call on a device at once
+
+// Once per device, with that device current: resolve the device address of the array and fill its table block.
+// Host-synchronous (a pageable cudaMemcpy), which is why the first call on a device belongs before any stream capture.
+int static_setup(int dev, StaticDev** out) {
+  if (dev < 0 || dev >= kStMaxDevices) { snprintf(g_errbuf, sizeof g_errbuf, "device ordinal %d is beyond the %d this entry point keeps state for", dev, kStMaxDevices); return FE_EINVAL; }
+  StaticDev& sd = g_static_dev[dev];
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!sd.ready) {
+    int major = 0, sms = 0;
+    FE_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    FE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10) { snprintf(g_errbuf, sizeof g_errbuf, "device %d is compute capability %d.x; libfe is built for sm_100a only", dev, major); return FE_EARCH; }
+    unsigned char* base = nullptr;
+    FE_CUDA(cudaGetSymbolAddress((void**)&base, fe_static_scratch));
+    if (!base) { snprintf(g_errbuf, sizeof g_errbuf, "cudaGetSymbolAddress returned a null address for the fixed scratch"); return FE_ECUDA; }
+    MathTabs host_tabs;                                     // 6.7 KB on the stack
+    memset(&host_tabs, 0, sizeof host_tabs);
+    build_tabs(&host_tabs);
+    FE_CUDA(cudaMemcpy(base, &host_tabs, sizeof(MathTabs), cudaMemcpyHostToDevice));
+    sd.base = base; sd.sm_count = sms; sd.ready = true;
+  }
+  *out = &sd;
+  return FE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fe_static_limits(int64_t* limits5) {
+  if (!limits5) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
+  limits5[0] = (int64_t)kStListMax; limits5[1] = (int64_t)kStTrigMax; limits5[2] = (int64_t)kStOutMax;
+  limits5[3] = (int64_t)kStPartialMax; limits5[4] = (int64_t)kStBytes;
+  return FE_OK;
+}
+
+int fe_omega_grid_static(const fe_model_params* params, int32_t N, double T,
+                         const double* q_xy, int32_t nq, const double* h_list, int32_t nh,
+                         const double* delta, int32_t nd, double* omega_dev, void* cuda_stream) {
+  if (!omega_dev) { snprintf(g_errbuf, sizeof g_errbuf, "omega_dev is NULL"); return FE_EINVAL; }
+  int rc = validate_params(params, N, T);
+  if (rc) return rc;
+  if ((rc = check_lists(q_xy, nq, h_list, nh, delta, nd))) return rc;
+  const int nb = nbands(*params);
+  if (nb == 3) { snprintf(g_errbuf, sizeof g_errbuf, "fe_omega_grid_static covers the one- and two-band models (the three-band model needs per-q band tables of 3 N^2 doubles)"); return FE_EINVAL; }
+  // ---- the fixed limits, checked before anything touches the device ----
+  const size_t nlist = (size_t)2 * nq + nh + nd, ntrig = (size_t)nq * N, nout = (size_t)nq * nh * nd;
+  if (nlist > kStListMax || ntrig > kStTrigMax || nout > kStOutMax) {
+    snprintf(g_errbuf, sizeof g_errbuf, "too large for the fixed scratch of fe_omega_grid_static: 2 nq + nh + nd = %zu (limit %zu), nq N = %zu (limit %zu), "
+             "nq nh nd = %zu (limit %zu); use fe_omega_grid, which allocates", nlist, kStListMax, ntrig, kStTrigMax, nout, kStOutMax);
+    return FE_EINVAL;
+  }
+  // ---- geometry of K1 (as fe_omega_grid in FE_EVAL_DIRECT mode: 4 x 4 register tile, 256 threads), k-chunks capped by the scratch ----
+  constexpr int tile = 1;
+  const int TH = kTiles[tile].th, TD = kTiles[tile].td;
+  KsumParams P;
+  P.mc = make_consts(*params);
+  P.T = T; P.neg_beta = -1.0 / T; P.window = 37.0 * T;
+  P.N = N; P.nq = nq; P.nh = nh; P.nd = nd;
+  P.debug_flags = 0;
+  P.ntile_h = (nh + TH - 1) / TH;
+  P.ntile_d = (nd + TD - 1) / TD;
+  int bxl = 8;                                        // 256 threads: all along kx when N allows it
+  while (bxl > 5 && (1 << (bxl - 1)) >= N) --bxl;
+  P.bx_log2 = bxl;
+  const int bx = 1 << bxl, by = kThreads >> bxl;
+  P.ncg = (N + bx - 1) / bx;
+  if ((size_t)P.ncg * nout > kStPartialMax) {
+    snprintf(g_errbuf, sizeof g_errbuf, "too large for the fixed scratch of fe_omega_grid_static: %d column groups x %zu outputs = %zu partial sums (limit %zu); "
+             "use fe_omega_grid, which allocates", P.ncg, nout, (size_t)P.ncg * nout, kStPartialMax);
+    return FE_EINVAL;
+  }
+  int dev = -1;
+  FE_CUDA(cudaGetDevice(&dev));
+  StaticDev* sd = nullptr;
+  if ((rc = static_setup(dev, &sd))) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const long long ntiles = (long long)nq * P.ntile_h * P.ntile_d;
+  long long nrs = ((long long)sd->sm_count * 2 * 24 + ntiles * P.ncg - 1) / (ntiles * P.ncg);
+  const long long cap_nrs = (long long)(kStPartialMax / ((size_t)P.ncg * nout));   // >= 1 (checked above)
+  if (nrs > cap_nrs) nrs = cap_nrs;
+  if (nrs > (N + by - 1) / by) nrs = (N + by - 1) / by;
+  if (nrs < 1) nrs = 1;
+  int rpc = (int)((N + nrs - 1) / nrs);
+  rpc = (rpc + by - 1) / by * by;
+  P.rows_per_chunk = rpc;
+  P.nrs = (N + rpc - 1) / rpc;
+  P.ksplit = P.ncg * P.nrs;
+  const long long grid_ll = ntiles * P.ksplit;
+  if (grid_ll > 2147483647LL) { snprintf(g_errbuf, sizeof g_errbuf, "grid too large"); return FE_EINVAL; }
+  // ---- carve the array ----
+  double* d_list = reinterpret_cast<double*>(sd->base + kStOffList);
+  double4* d_col = reinterpret_cast<double4*>(sd->base + kStOffCol);
+  double4* d_row = reinterpret_cast<double4*>(sd->base + kStOffRow);
+  double* d_spart = reinterpret_cast<double*>(sd->base + kStOffSpart);
+  double* d_partial = reinterpret_cast<double*>(sd->base + kStOffPartial);
+  // ---- lists: assembled on the stack, copied from pageable memory (the copy call returns once the source may be reused) ----
+  double hs[kStListMax];
+  memcpy(hs, q_xy, sizeof(double) * 2 * nq);
+  memcpy(hs + 2 * nq, h_list, sizeof(double) * nh);
+  for (int i = 0; i < nd; ++i) hs[2 * nq + nh + i] = delta[i] * delta[i];
+  FE_CUDA(cudaMemcpyAsync(d_list, hs, nlist * sizeof(double), cudaMemcpyHostToDevice, st));
+  const double* d_q = d_list;
+  P.h = d_list + 2 * nq; P.d2 = d_list + 2 * nq + nh; P.htile = nullptr;
+  P.coltab = d_col; P.rowtab = d_row; P.tabs = reinterpret_cast<const MathTabs*>(sd->base); P.partial = d_partial;
+  // ---- K0, KS, K1, K2.  Each of them writes every scratch word that a later one reads (all nq N table entries, all nq x
+  // nschunk constant sums, all ksplit x nout partial sums, empty chunks included), so nothing has to start at zero and what
+  // an earlier, larger call left behind is never read. ----
+  fe_trig_kernel<<<(N * nq + 255) / 256, 256, 0, st>>>(N, nq, d_q, d_col, d_row);
+  FE_CUDA(cudaGetLastError());
+  int nschunk = N < kSChunksMax ? N : kSChunksMax;
+  const int srpc = (N + nschunk - 1) / nschunk;
+  nschunk = (N + srpc - 1) / srpc;
+  {
+    dim3 g(nschunk, nq);
+    if (nb == 1) fe_ssum_kernel<1><<<g, kThreads, 0, st>>>(P.mc, N, srpc, d_col, d_row, d_spart);
+    else         fe_ssum_kernel<2><<<g, kThreads, 0, st>>>(P.mc, N, srpc, d_col, d_row, d_spart);
+    FE_CUDA(cudaGetLastError());
+  }
+  FE_CUDA(launch_ksum(tile, nb, params->form_factor, FE_EVAL_DIRECT, (int)grid_ll, st, P));
+  const double condc = params->cond_mult * (double)N * (double)N / params->U;
+  fe_finish_kernel<<<(unsigned)((nout + 255) / 256), 256, 0, st>>>(nq, nh, nd, P.ksplit, nschunk, condc, d_partial, d_spart, P.d2, omega_dev);
+  FE_CUDA(cudaGetLastError());
+  return FE_OK;
 }
 
 }  // extern "C"

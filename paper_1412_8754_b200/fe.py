@@ -19,7 +19,7 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 # include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
-               "fe_get_launch_count", "fe_get_slot_counts", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
+               "fe_get_launch_count", "fe_get_slot_counts", "fe_omega_grid_static", "fe_static_limits", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math",
                  "fe_set_chi_table_budget", "fe_debug_sym_index", "fe_debug_coop_occupancy"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
@@ -87,6 +87,8 @@ def lib():
     L.fe_coop_shape_info.argtypes = [C.c_int32, ip]
     L.fe_fp64_peak_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_float), dp, vp]
     L.fe_debug_math.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp]
+    L.fe_omega_grid_static.argtypes = [C.POINTER(ModelParams), C.c_int32, C.c_double, dp, C.c_int32, dp, C.c_int32, dp, C.c_int32, vp, vp]
+    L.fe_static_limits.argtypes = [C.POINTER(C.c_int64)]
     L.fe_destroy.argtypes = [vp]
     L.fe_destroy.restype = None
     L.fe_strerror.argtypes = [C.c_int]
@@ -173,6 +175,30 @@ def fp64_peak_probe(blocks=148 * 16, iters=1 << 16, stream=None):
     ms, cnt = C.c_float(), C.c_double()
     _check(lib().fe_fp64_peak_probe(blocks, iters, C.byref(ms), C.byref(cnt), _stream(stream)))
     return cnt.value / (ms.value * 1e-3), ms.value
+
+
+def static_limits():
+    """Limits of omega_grid_static (fe_static_limits): dict(list, trig, out, partial, bytes).  No CUDA call."""
+    a = (C.c_int64 * 5)()
+    _check(lib().fe_static_limits(a))
+    return dict(list=a[0], trig=a[1], out=a[2], partial=a[3], bytes=a[4])
+
+
+def omega_grid_static(params: dict, N: int, T: float, q, h, delta, out, stream=None):
+    """Omega[iq, ih, id] on a small grid through fe_omega_grid_static, the entry point for callers that cannot let the
+    library allocate: no handle, and all working memory in a fixed array inside libfe.so (limits: static_limits()).
+
+    Nothing is allocated here either, so `out` is required: a contiguous float64 CUDA tensor with nq*nh*nd elements that
+    the caller made while it still could.  All calls on a device share the library's one scratch array; keep them on one
+    stream (include/fe.h says what happens otherwise).  Returns `out`; asynchronous on `stream` (default: current)."""
+    import torch
+    q, h, d = _f64(q, (-1, 2)), _f64(h), _f64(delta)
+    shape = (q.shape[0], h.shape[0], d.shape[0])
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == int(np.prod(shape))
+    p = make_params(params)
+    _check(lib().fe_omega_grid_static(C.byref(p), int(N), float(T), _dptr(q), shape[0], _dptr(h), shape[1], _dptr(d), shape[2],
+                                      C.c_void_p(out.data_ptr()), _stream(stream)))
+    return out
 
 
 class FreeEnergy:
