@@ -192,11 +192,30 @@ def oracle_sample(w, T, n_delta, nthreads=None, columns=1):
     ids = np.unique(np.linspace(0, w.nd - 1, n_delta).round().astype(int))
     cols = [(w.nq // 2, w.nh // 2), (w.nq // 4, (3 * w.nh) // 4), ((3 * w.nq) // 4, w.nh // 4)][:columns]
     t0 = time.perf_counter()
-    for iq, ih in cols:
-        O.omega_column(w.params, w.N, T, w.q[iq], w.h[ih], w.delta[ids])
+    vals = [O.omega_column(w.params, w.N, T, w.q[iq], w.h[ih], w.delta[ids]) for iq, ih in cols]
     dt = time.perf_counter() - t0
     evals = w.N * w.N * len(ids) * len(cols)
+    oracle_sample.last = dict(T=T, cols=cols, ids=ids, values=vals)       # bench.py's parity figure reuses these columns
     return evals / dt, dt, len(ids), O.num_threads(), cols
+
+
+def parity_vs_oracle_columns(om_gpu, col_idx, cols):
+    """Parity figure of the Omega bench line: the oracle columns cpu_baseline computed anyway (cols = oracle_sample.last)
+    against ONE untimed fe_omega_grid launch of exactly the shape the timed loop runs (om_gpu[row, ih, id], row r = q number
+    col_idx[r] of the workload).  Elementwise max relative error; argmin compared when the whole Delta list was sampled."""
+    ids, errs, arg_eq, ncmp = cols["ids"], [], [], 0
+    pos = {int(g): r for r, g in enumerate(col_idx)}
+    for (iq, ih), ref in zip(cols["cols"], cols["values"]):
+        if iq not in pos or pos[iq] >= om_gpu.shape[0]:
+            continue                                     # a q-value another rank owns
+        got = om_gpu[pos[iq], ih]
+        errs.append(float(np.max(np.abs(got[ids] - ref) / np.abs(ref))))
+        ncmp += 1
+        if len(ids) == om_gpu.shape[2]:
+            arg_eq.append(int(np.argmin(got)) == int(np.argmin(ref)))
+    return {"max_rel_err": max(errs) if errs else None, "columns": ncmp, "delta_values_per_column": int(len(ids)), "T": cols["T"],
+            "argmin_equal": (all(arg_eq) if arg_eq else None), "tolerance": 1e-12,
+            "what": "oracle columns of cpu_baseline vs one untimed fe_omega_grid launch of the timed shape (all q of the step, same eval mode)"}
 
 
 def cpu_baseline(w, T, n_delta_all, n_delta_one):
@@ -204,6 +223,7 @@ def cpu_baseline(w, T, n_delta_all, n_delta_one):
     ncores = os.cpu_count() or 1
     v1, dt1, nd1, th1, cols1 = oracle_sample(w, T, n_delta_one, nthreads=1)
     va, dta, nda, tha, colsa = oracle_sample(w, T, n_delta_all, nthreads=ncores, columns=2)
+    cpu_baseline.columns = oracle_sample.last
     return {"value": va, "unit": UNIT, "cores": tha, "kind": "oracle", "seconds": dta, "cpu_model": cpu_model(),
             "sample": (f"{len(colsa)} of {w.nq * w.nh} (q,h) columns of {w.name} {colsa} x {nda} of {w.nd} Delta, "
                        f"full {w.N}x{w.N} k-sum, T={T}, OpenMP over Delta"),
@@ -295,9 +315,9 @@ def apply_counts(roof, counts, status, labels, k_ms, units_per_launch, unit_name
     per_label = {l: {"fp64_inst_per_" + unit_name: counts[l]["inst"] / units_per_launch,
                      "dadd_dmul_dfma_per_" + unit_name: [counts[l][o] / units_per_launch for o in FP64_OPS],
                      "ncu_fp64_pipe_active_pct": counts[l]["pipe_pct"], "ncu_launch_ms": counts[l]["ncu_ms"],
-                     "dram_bytes": counts[l]["dram_bytes"]} for l in sorted(set(labels))}
-    roof["counts"] = {"source": counts[labels[0]]["file"], "kernel": counts[labels[0]]["kernel"], "grid": counts[labels[0]]["grid"],
-                      "per_launch": per_label}
+                     "dram_bytes": counts[l]["dram_bytes"], "kernel": counts[l]["kernel"], "grid": counts[l]["grid"]}
+                 for l in sorted(set(labels))}
+    roof["counts"] = {"source": counts[labels[0]]["file"], "per_launch": per_label}
     tr = [counts[l]["dram_bytes"] for l in labels if counts[l]["dram_bytes"]]
     roof["traffic"] = sum(tr) / len(tr) if tr else None
     if status is not None:
@@ -577,14 +597,21 @@ def main():
             band_evals = be
             li = F.last_launch_info()
             tiles_by_T[f"T={step_T[-1]:g}"] = f"{li['th']}x{li['td']}"
-            if args.mode in ("coop", "coop_eo"):
-                c = F.slot_counts()                     # device -> host read of four counters, outside the events
-                tot = c["dense"] + c["a_dominated"] + c["b_dominated"]
-                slot_kinds[f"T={step_T[-1]:g}"] = {k: v / tot for k, v in c.items()}
     barrier()
     t_wall = time.perf_counter() - t_wall0
     launches = F.launch_count() - launches0
     clocks = sampler.stop()
+    if args.mode in ("coop", "coop_eo") and nq_rank:
+        # what the launches were made of: the kernel counts its slot kinds with global atomics, so the counters are OFF in
+        # every timed launch above and collected here in one extra, untimed step per temperature (same inputs: the
+        # classification does not depend on timing)
+        F.enable_slot_counts(True)
+        for s in range(len(temps)):
+            one_step(args.warmup + s)
+            c = F.slot_counts()                         # waits for the launch, reads five counters
+            tot = c["dense"] + c["a_dominated"] + c["b_dominated"]
+            slot_kinds[f"T={temps[(args.warmup + s) % len(temps)]:g}"] = {k: v / tot for k, v in c.items()}
+        F.enable_slot_counts(False)
     idx_check = int(res[0].sum().item()) if res is not None else 0      # device->host read of the step's result
 
     total_ms = sum(step_ms)
@@ -712,7 +739,7 @@ def main():
     roofline.update({"avg_launch_ms": k_ms, "median_launch_ms": statistics.median(ksum_ms), "band_evals_per_launch": band_evals,
                      "kernel_share_of_step": sum(ksum_ms) / total_ms})
     if slot_kinds:
-        roofline["slot_kinds"] = {"what": "fractions of the (k, band, block tile) slots of a timed launch, counted by the kernel in this run: "
+        roofline["slot_kinds"] = {"what": "fractions of the (k, band, block tile) slots of one launch per temperature, counted by the kernel in an extra untimed step of this run (the counters are off in the timed launches): "
                                           "dense slots (and padding, relative to the same total) run through the pair products, "
                                           "dominated slots are summed without exponentials", **slot_kinds}
     if sp_mode:
@@ -722,9 +749,15 @@ def main():
         counts, status = kernel_counts(f"omega/{args.mode}/{w.name}/q{nq_step}", "fe_ksum", hashes)
         apply_counts(roofline, counts, status, [f"T={x:g}" for x in step_T], ksum_ms, band_evals, "band_eval")
 
-    cpu = None
+    cpu, parity = None, None
     if not args.no_cpu_baseline:
         cpu = cpu_baseline(w, temps[0], args.cpu_baseline_deltas, 32)
+        if not sp_mode and nq_rank:
+            F.set_temperature(temps[0])                 # one untimed launch of the timed shape at the oracle's temperature
+            F.omega_grid(q_of(0), w.h, w.delta, out=omega, stream=stream)
+            torch.cuda.synchronize()
+            parity = parity_vs_oracle_columns(omega.cpu().numpy(), col_idx[:nq_step] % max(len(w.q), 1), cpu_baseline.columns)
+            parity["launch"] = F.last_launch_info()
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "ms_per_step_median": statistics.median(step_ms),
@@ -737,7 +770,7 @@ def main():
                     "steps": e2e_steps, "api": "fe_scan_host (host buffers in/out, synchronous)" +
                     (" + all_gather of the minima" if world > 1 else "")},
             "gpu_launches": launches, "wall_s_timed_region": t_wall, "clocks": clocks, "source_hash": hashes[0],
-            "roofline": roofline, "dense_variant": dense, "symmetric_variant": symv, "cpu_baseline": cpu, "result_check": idx_check}
+            "roofline": roofline, "dense_variant": dense, "symmetric_variant": symv, "cpu_baseline": cpu, "parity": parity, "result_check": idx_check}
     if sp_mode:
         line["verified_per_step"] = verified[-args.steps:]
     print(json.dumps(line), flush=True)

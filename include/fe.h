@@ -151,8 +151,9 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
  * Asynchronous on cuda_stream; deterministic.  With fe_enable_timing the k-sum kernel of this call is the one
  * fe_get_timing reports (its second value is then the number of (k, q, e, f) pair terms).  Three-band model: q-values on
  * the k-grid read the unshifted band table at a shifted index; q-values off the grid need a table each (3 N^2 doubles),
- * so the list is worked through in consecutive slices whose tables fit ~2 GB of scratch (fe_get_timing then reports the
- * last slice).               */
+ * so the list is worked through in consecutive slices whose tables fit ~2 GB of scratch; fe_get_timing then reports the
+ * pair terms of ALL slices and the time from the start of the first slice's k-sum kernel to the end of the last one's (the
+ * table and finishing kernels of the slices in between are inside that interval).               */
 int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream);
 
 /* The paper's single-precision builds: Omega on the full grid with every per-term
@@ -252,18 +253,22 @@ int fe_static_limits(int64_t* limits5);
 int fe_enable_timing(fe_handle* h, int32_t on);
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals);
 
-/* What the most recent TIMED cooperative k-sum launch (FE_EVAL_COOP / FE_EVAL_COOP_EO with fe_enable_timing on) was made
- * of: counts5 = {dense, A-dominated (summed as square roots per Delta_j), B-dominated, padding, A-dominated (summed through
- * the moment series)} (k, band) slots, each counted once per block tile it was classified for (a slot of a 64 x 128 block
- * tile stands for 8192 (h, Delta) pairs).  Dense and padding slots run through the pair products, dominated slots are
- * summed without exponentials (FE_EVAL_COOP_EO; FE_EVAL_COOP has none).  HOST doubles; call after synchronising the
- * stream (the call copies five counters from the device).  FE_EINVAL if there is none. */
+/* What a cooperative k-sum launch (FE_EVAL_COOP / FE_EVAL_COOP_EO) was made of.  fe_enable_slot_counts(h, 1) makes every
+ * following launch count its (k, band) slots by kind -- a few global atomics per group of k-points, so leave it OFF (the
+ * default) in launches whose duration is being measured; fe_enable_timing does not switch it on.  fe_get_slot_counts then
+ * returns, for the most recent counted launch, counts5 = {dense, A-dominated (summed as square roots per Delta_j),
+ * B-dominated, padding, A-dominated (summed through the moment series)} slots, each counted once per block tile it was
+ * classified for (a slot of a 64 x 128 block tile stands for 8192 (h, Delta) pairs).  Dense and padding slots run through
+ * the pair products, dominated slots are summed without exponentials (FE_EVAL_COOP_EO; FE_EVAL_COOP has none).  HOST
+ * doubles.  The call copies the five counters on the stream of that launch and waits for that stream.  FE_EINVAL if there
+ * is no counted launch. */
+int fe_enable_slot_counts(fe_handle* h, int32_t on);
 int fe_get_slot_counts(fe_handle* h, double* counts5);
 
 /* Launch configuration of the most recent k-sum kernel: info6 = {TH, TD, ksplit, grid blocks, eval mode actually
  * used, rows per k-chunk}; for FE_EVAL_COOP / FE_EVAL_COOP_EO: {WH, WD, ksplit, grid blocks, mode, k-points per chunk};
  * after fe_omega_grid_sp the mode entry is 101 (SP) or 102 (SPFM); after fe_pair_susceptibility
- * {nb, nb, k-chunks, grid blocks, -1, k-points per chunk}.  Host-only. */
+ * {nb, nb, k-chunks, grid blocks (summed over the slices of the call), -1, k-points per chunk}.  Host-only. */
 int fe_get_last_launch_info(fe_handle* h, int32_t* info6);
 
 /* Number of kernel launches this handle has issued since creation (all kernels of this library). */

@@ -99,12 +99,14 @@ struct fe_handle {
   int next_slot = 0;
   // timing
   bool timing = false;
+  bool slot_counts = false;    // fe_enable_slot_counts: the cooperative kernel counts its slot kinds (atomics; off in timed runs)
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timing_valid = false;
   double last_band_evals = 0;
   int32_t last_info[6] = {0, 0, 0, 0, 0, 0};   // th, td, ksplit, grid, mode, rows_per_chunk
   unsigned long long* d_kinds = nullptr;       // 5 slot-kind counters of the most recent timed K1c launch
   bool kinds_valid = false;
+  cudaStream_t kinds_stream = nullptr;         // stream of that launch: fe_get_slot_counts copies on it and waits for it
   int64_t launches = 0;
 };
 
@@ -589,11 +591,12 @@ int omega_grid_impl(fe_handle* h, const double* q_xy, int32_t nq, const double* 
     CP.partial = h->d_partial; CP.etab = h->d_etab;
     CP.kind_counts = nullptr;
     h->kinds_valid = false;
-    if (h->timing) {
+    if (h->slot_counts) {
       if (!h->d_kinds) FE_CUDA(cudaMalloc((void**)&h->d_kinds, 5 * sizeof(unsigned long long)));
       FE_CUDA(cudaMemsetAsync(h->d_kinds, 0, 5 * sizeof(unsigned long long), st));
       CP.kind_counts = h->d_kinds;
       h->kinds_valid = true;
+      h->kinds_stream = st;
     }
   }
   if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
@@ -816,7 +819,18 @@ int fe_argmin_q(fe_handle* h, const double* omega_dev, int32_t nq, int32_t nh, i
   return FE_OK;
 }
 
-static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
+// q on the k-grid?  (then E(k + q) is the unshifted band table read at a shifted index: no table of its own.)  The ONE
+// predicate both the slicing of fe_pair_susceptibility and the shift codes of chi_slice use; *sx, *sy = grid shift in [0, N).
+static bool chi_q_on_grid(const double* q, int N, long long* sx, long long* sy) {
+  const double mx = q[0] * N / (2.0 * 3.14159265358979323846), my = q[1] * N / (2.0 * 3.14159265358979323846);
+  const double rx = nearbyint(mx), ry = nearbyint(my);
+  if (!(fabs(mx - rx) <= 1e-9 && fabs(my - ry) <= 1e-9 && fabs(rx) < 1e15 && fabs(ry) < 1e15)) return false;
+  if (sx) *sx = (((long long)rx % N) + N) % N;
+  if (sy) *sy = (((long long)ry % N) + N) % N;
+  return true;
+}
+
+static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream, bool first_slice) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = h->N, nb = h->nb, nbb = nb * nb;
   if (int rcd = check_device(h)) return rcd;
@@ -826,15 +840,10 @@ static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, do
   for (int i = 0; i < 2 * nq; ++i) hs[i] = -q_xy[i];          // tables of k - (-q) = k + q; E, eta even: = -k - q
   int noff = 0;                                               // q-values off the k-grid: they need a band table each
   for (int i = 0; i < nq; ++i) {                              // q on the k-grid: shift code sx + sy N, else -(table index)
-    const double mx = q_xy[2 * i] * N / (2.0 * 3.14159265358979323846), my = q_xy[2 * i + 1] * N / (2.0 * 3.14159265358979323846);
-    const double rx = nearbyint(mx), ry = nearbyint(my);
+    long long sx = 0, sy = 0;
     double code = -(double)(1 + noff);
-    if (fabs(mx - rx) <= 1e-9 && fabs(my - ry) <= 1e-9 && fabs(rx) < 1e15 && fabs(ry) < 1e15) {
-      const long long sx = (((long long)rx % N) + N) % N, sy = (((long long)ry % N) + N) % N;
-      code = (double)(sx + sy * (long long)N);
-    } else {
-      ++noff;
-    }
+    if (chi_q_on_grid(q_xy + 2 * i, N, &sx, &sy)) code = (double)(sx + sy * (long long)N);
+    else ++noff;
     hs[2 * nq + i] = code;
   }
   FE_CUDA(cudaMemcpyAsync(ds, hs, (size_t)3 * nq * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -873,7 +882,7 @@ static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, do
   }
   const ModelConsts mc = make_consts(h->p);
   dim3 grid((unsigned)nchunk, (unsigned)nq);
-  if (h->timing) FE_CUDA(cudaEventRecord(h->ev0, st));
+  if (h->timing && first_slice) FE_CUDA(cudaEventRecord(h->ev0, st));
   const int form = h->p.form_factor;
 #define FE_CHI(NB_, F_) fe_chi_kernel<NB_, F_><<<grid, kThreads, 0, st>>>(mc, h->T, hz, N, nq, kc, h->d_coltab, h->d_rowtab, h->d_etab, ds + 2 * nq, h->d_tabs, h->d_partial)
   if (nb == 1) { if (form == 0) FE_CHI(1, 0); else FE_CHI(1, 1); }
@@ -885,9 +894,10 @@ static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, do
   if (h->timing) {
     FE_CUDA(cudaEventRecord(h->ev1, st));
     h->timing_valid = true;
-    h->last_band_evals = (double)nk * nq * nbb;
+    h->last_band_evals = (first_slice ? 0.0 : h->last_band_evals) + (double)nk * nq * nbb;
   }
-  h->last_info[0] = nb; h->last_info[1] = nb; h->last_info[2] = (int32_t)nchunk; h->last_info[3] = (int32_t)(nchunk * nq);
+  h->last_info[0] = nb; h->last_info[1] = nb; h->last_info[2] = (int32_t)nchunk;
+  h->last_info[3] = (first_slice ? 0 : h->last_info[3]) + (int32_t)(nchunk * nq);                 // blocks of all slices
   h->last_info[4] = -1; h->last_info[5] = (int32_t)(kc < 2147483647ULL ? kc : 2147483647ULL);
   const int nout = nq * nbb;
   fe_chi_finish_kernel<<<(nout + 255) / 256, 256, 0, st>>>(nout, (int)nchunk, 1.0 / ((double)N * (double)N), h->d_partial, chi_dev);
@@ -896,17 +906,11 @@ static int chi_slice(fe_handle* h, const double* q_xy, int32_t nq, double hz, do
   return FE_OK;
 }
 
-// q on the k-grid?  (then E(k + q) is the unshifted band table read at a shifted index: no table of its own)
-static bool chi_q_on_grid(const double* q, int N) {
-  const double mx = q[0] * N / (2.0 * 3.14159265358979323846), my = q[1] * N / (2.0 * 3.14159265358979323846);
-  return fabs(mx - nearbyint(mx)) <= 1e-9 && fabs(my - nearbyint(my)) <= 1e-9 && fabs(mx) < 1e15 && fabs(my) < 1e15;
-}
-
 int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double hz, double* chi_dev, void* cuda_stream) {
   if (!h || !q_xy || !chi_dev) { snprintf(g_errbuf, sizeof g_errbuf, "handle, q_xy or chi_dev is NULL"); return FE_EINVAL; }
   if (nq < 1 || nq > kMaxQ || !isfinite(hz)) { snprintf(g_errbuf, sizeof g_errbuf, "nq must be in [1, %d], hz finite", kMaxQ); return FE_EINVAL; }
   for (int i = 0; i < 2 * nq; ++i) if (!isfinite(q_xy[i])) { snprintf(g_errbuf, sizeof g_errbuf, "q[%d] not finite", i); return FE_EINVAL; }
-  if (h->nb < 3) return chi_slice(h, q_xy, nq, hz, chi_dev, cuda_stream);
+  if (h->nb < 3) return chi_slice(h, q_xy, nq, hz, chi_dev, cuda_stream, true);
   // Three-band model: every q OFF the k-grid needs a band table of its own (24 MB at N = 1024).  The q list is processed
   // in consecutive slices that hold at most `maxoff` such q-values, so the table scratch stays below ~2 GB (chi_table_budget) whatever the
   // size of the map (a 48 x 48 off-grid map would otherwise need 55 GB); slices reuse the scratch in stream order.
@@ -918,11 +922,11 @@ int fe_pair_susceptibility(fe_handle* h, const double* q_xy, int32_t nq, double 
   while (q0 < nq) {
     int q1 = q0, noff = 0;
     while (q1 < nq) {
-      const int off = chi_q_on_grid(q_xy + 2 * q1, h->N) ? 0 : 1;
+      const int off = chi_q_on_grid(q_xy + 2 * q1, h->N, nullptr, nullptr) ? 0 : 1;
       if (noff + off > maxoff) break;
       noff += off; ++q1;
     }
-    const int rc = chi_slice(h, q_xy + 2 * q0, q1 - q0, hz, chi_dev + (size_t)q0 * nbb, cuda_stream);
+    const int rc = chi_slice(h, q_xy + 2 * q0, q1 - q0, hz, chi_dev + (size_t)q0 * nbb, cuda_stream, q0 == 0);
     if (rc) return rc;
     q0 = q1;
   }
@@ -1052,6 +1056,13 @@ int fe_enable_timing(fe_handle* h, int32_t on) {
   return FE_OK;
 }
 
+int fe_enable_slot_counts(fe_handle* h, int32_t on) {
+  if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
+  h->slot_counts = on != 0;
+  h->kinds_valid = false;
+  return FE_OK;
+}
+
 int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
   if (!h) { snprintf(g_errbuf, sizeof g_errbuf, "handle is NULL"); return FE_EINVAL; }
   if (!h->timing_valid) { snprintf(g_errbuf, sizeof g_errbuf, "no timed launch recorded"); return FE_EINVAL; }
@@ -1064,9 +1075,11 @@ int fe_get_timing(fe_handle* h, float* ksum_ms, double* band_evals) {
 
 int fe_get_slot_counts(fe_handle* h, double* counts5) {
   if (!h || !counts5) { snprintf(g_errbuf, sizeof g_errbuf, "NULL argument"); return FE_EINVAL; }
-  if (!h->kinds_valid || !h->d_kinds) { snprintf(g_errbuf, sizeof g_errbuf, "no timed cooperative k-sum launch recorded"); return FE_EINVAL; }
+  if (!h->kinds_valid || !h->d_kinds) { snprintf(g_errbuf, sizeof g_errbuf, "no counted cooperative k-sum launch recorded (fe_enable_slot_counts)"); return FE_EINVAL; }
   unsigned long long c[5];
-  FE_CUDA(cudaMemcpy(c, h->d_kinds, sizeof c, cudaMemcpyDeviceToHost));
+  // on the stream of the counted launch, then wait for it: a non-blocking user stream is not ordered with the default stream
+  FE_CUDA(cudaMemcpyAsync(c, h->d_kinds, sizeof c, cudaMemcpyDeviceToHost, h->kinds_stream));
+  FE_CUDA(cudaStreamSynchronize(h->kinds_stream));
   for (int i = 0; i < 5; ++i) counts5[i] = (double)c[i];
   return FE_OK;
 }

@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
       const int nl = last_group ? 0 : nfront - nsub * SLOTS;
       carry_state = nl | ((rob && nl > 0) ? 0x100 : 0) | ((nsub * SLOTS) << 9);
     }
-    if (P.kind_counts != nullptr && tid == 0) {              // diagnostics only (fe_enable_timing): what the launch was made of
+    if (P.kind_counts != nullptr && tid == 0) {              // diagnostics only (fe_enable_slot_counts): what the launch was made of
       if (ndense) atomicAdd(P.kind_counts + 0, (unsigned long long)ndense);
       if (ndom) atomicAdd(P.kind_counts + 1, (unsigned long long)ndom);
       if (ndomB) atomicAdd(P.kind_counts + 2, (unsigned long long)ndomB);
@@ -822,16 +822,29 @@ __global__ void __launch_bounds__(NW * 32, MINB) fe_ksum_coop_kernel(const CoopP
     double sumB = 0.0;                                         // B-dominated slots, fixed order over the partial sums
 #pragma unroll
     for (int hf = 0; hf < NT / WH; ++hf) sumB += accB_s[hf * WH + thx * TH + i];
+    double v[TD];
 #pragma unroll
     for (int j = 0; j < TD; ++j) {
-      const int id = td * WD + tdx * TD + j;
       const int hi = __double2hiint(accP[i][j]);
       const int ex = (hi >> 20) - 1023;
       const double mant = __hiloint2double(hi - (ex << 20), __double2loint(accP[i][j]));
       const double ed = (double)accEc + (double)(myE[(i * TD + j) * NT] - 1023 * nrenorm + ex);
       const double lnz = fma(ed, LN2_HI, fma(ed, LN2_LO, log(mant)));
-      if (ih < P.nh && id < P.nd)
-        P.partial[(size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id] = weight * fma(P.T, lnz, accR_s[tdx * TD + j] + sumB);
+      v[j] = weight * fma(P.T, lnz, accR_s[tdx * TD + j] + sumB);
+    }
+    // a thread's TD Delta values are consecutive in memory: one 32-byte store per (thread, h) when the row length keeps
+    // them 32-byte aligned (nd % 4 == 0; the group is then wholly inside or outside the list), else one double at a time
+    const int id0 = td * WD + tdx * TD;
+    double* dst = P.partial + (size_t)chunk * nout + ((size_t)iq * P.nh + ih) * P.nd + id0;
+    if (ih < P.nh) {
+      if (TD == 4 && (P.nd & 3) == 0) {
+        if (id0 < P.nd)
+          asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" :: "l"(dst), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[TD - 1]) : "memory");
+      } else {
+#pragma unroll
+        for (int j = 0; j < TD; ++j)
+          if (id0 + j < P.nd) dst[j] = v[j];
+      }
     }
   }
 }

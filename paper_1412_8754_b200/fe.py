@@ -19,7 +19,7 @@ EVAL_FACTORED, EVAL_DIRECT, EVAL_WINDOWED, EVAL_COOP, EVAL_COOP_EO = 0, 1, 2, 3,
 # include/fe.h (the boundary) and include/fe_debug.h (test / tuning hooks)
 EXPORTS_API = ["fe_create", "fe_set_temperature", "fe_set_eval_mode", "fe_omega_grid", "fe_argmin", "fe_argmin_q", "fe_pair_susceptibility",
                "fe_omega_grid_sp", "fe_scan_verified", "fe_scan_host", "fe_enable_timing", "fe_get_timing", "fe_get_last_launch_info",
-               "fe_get_launch_count", "fe_get_slot_counts", "fe_omega_grid_static", "fe_static_limits", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
+               "fe_get_launch_count", "fe_get_slot_counts", "fe_enable_slot_counts", "fe_omega_grid_static", "fe_static_limits", "fe_set_symmetry", "fe_get_last_symmetry", "fe_fp64_peak_probe", "fe_build_source_hash", "fe_destroy", "fe_strerror"]
 EXPORTS_DEBUG = ["fe_set_tuning", "fe_tile_info", "fe_set_debug_flags", "fe_set_coop_shape", "fe_coop_shape_info", "fe_debug_math",
                  "fe_set_chi_table_budget", "fe_debug_sym_index", "fe_debug_coop_occupancy"]
 EXPORTS = EXPORTS_API + EXPORTS_DEBUG
@@ -75,6 +75,7 @@ def lib():
     L.fe_get_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.fe_get_last_launch_info.argtypes = [vp, ip]
     L.fe_get_slot_counts.argtypes = [vp, dp]
+    L.fe_enable_slot_counts.argtypes = [vp, C.c_int32]
     L.fe_debug_sym_index.argtypes = [C.c_int32, C.c_int32, C.c_int64, ip, ip, C.POINTER(C.c_int64)]
     L.fe_debug_coop_occupancy.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, ip]
     L.fe_set_symmetry.argtypes = [vp, C.c_int32]
@@ -256,6 +257,10 @@ class FreeEnergy:
     def enable_timing(self, on=True):
         _check(lib().fe_enable_timing(self._h, 1 if on else 0))
 
+    def enable_slot_counts(self, on=True):
+        """Count slot kinds in the following cooperative launches (atomics in the kernel: keep off while timing)."""
+        _check(lib().fe_enable_slot_counts(self._h, 1 if on else 0))
+
     def last_ksum(self):
         """(ms, band_evals) of the most recent k-sum launch; call after synchronising the stream."""
         ms, be = C.c_float(), C.c_double()
@@ -268,8 +273,8 @@ class FreeEnergy:
         return dict(th=a[0], td=a[1], ksplit=a[2], grid=a[3], mode=a[4], rows_per_chunk=a[5])
 
     def slot_counts(self):
-        """{dense, a_dominated (= list + series), a_series, b_dominated, padding} slot counts of the most recent timed
-        cooperative k-sum launch."""
+        """{dense, a_dominated (= list + series), a_series, b_dominated, padding} slot counts of the most recent cooperative
+        k-sum launch made with enable_slot_counts on."""
         a = (C.c_double * 5)()
         _check(lib().fe_get_slot_counts(self._h, a))
         return dict(dense=a[0], a_dominated=a[1] + a[4], a_series=a[4], b_dominated=a[2], padding=a[3])

@@ -2,7 +2,7 @@
 
 Calls ONLY oracle/ (never the CUDA path).  The GPU parity tests at full size (configs 3-5) compare against
 these stored values so that the GPU box does not spend minutes of host time re-deriving them; the samples are
-WHOLE (q, h) columns (all Delta, full k-sum), so the argmin check against the oracle is meaningful: 12 columns of
+WHOLE (q, h) columns (all Delta, full k-sum), so the argmin check against the oracle is meaningful: 64 columns of
 config 3, 16 per temperature of config 4, 4 per seed for seeds 1-3 of config 5 (each seed is its own
 run with its own perturbed hoppings, stored with the run).  Floats are stored with repr() (exact round trip).
 
@@ -24,7 +24,7 @@ from paper_1412_8754_b200 import workloads as W      # noqa: E402
 HERE = os.path.dirname(os.path.abspath(__file__))
 
 PLAN = {            # cfg: (number of (q,h) columns per run, Delta indices per column or None = all)
-    3: (12, None),
+    3: (64, None),       # 64 columns of config 3
     4: (16, None),
     5: (4, None),
 }

@@ -639,7 +639,7 @@ def test_full_size_properties_in_bench_launch_configuration(fe):
 
 
 def test_slot_counters_and_moment_series(fe, oracle):
-    """fe_get_slot_counts: every (k, band, block tile) slot of a timed launch is classified exactly once; the dense variant has
+    """fe_get_slot_counts: every (k, band, block tile) slot of a counted launch (fe_enable_slot_counts) is classified exactly once; the dense variant has
     no dominated slots; at low T most A-dominated slots go through the moment series (Delta^2 g <= s^2 / 16 over the tile),
     and a grid with large Delta (eps > 1/16 near the Fermi surface) uses both the series and the square-root list."""
     import torch
@@ -652,9 +652,13 @@ def test_slot_counters_and_moment_series(fe, oracle):
                 F.set_eval_mode(mode)
                 F.set_coop_shape(1)
                 F.enable_timing(True)
+                with pytest.raises(fe.FeError):
+                    F.omega_grid(w.q, w.h, w.delta)
+                    F.slot_counts()                      # timing alone does not count: nothing recorded
+                F.enable_slot_counts(True)
                 om = F.omega_grid(w.q, w.h, w.delta)
+                c = F.slot_counts()                      # waits for the launch itself (no synchronize here on purpose)
                 torch.cuda.synchronize()
-                c = F.slot_counts()
                 info = F.last_launch_info()
             assert max_rel(om.cpu().numpy(), ref) < RTOL
             tiles = w.nq * -(-w.nh // info["th"]) * -(-w.nd // info["td"])
@@ -858,9 +862,10 @@ def _golden_runs(cfg):
 @pytest.mark.parametrize("mode", [4, 3, 0])
 @pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_full_size_configs_sampled_parity(fe, cfg, mode):
-    """Whole oracle (q, h) columns (all Delta, full k-sum) of configs 3-5 -- 12 / 16 per T / 4 per seed for seeds 1-3 --
-    against the device in the launch configuration bench.py times: Omega elementwise at 1e-12 and the per-column minimum
-    (index, Delta*, Omega*) against the oracle's (reading G11 for near-ties)."""
+    """Whole oracle (q, h) columns (all Delta, full k-sum) of configs 3-5 -- 64 / 16 per T / 4 per seed for seeds 1-3 --
+    against the device, ONE q per call on the config's full (h, Delta) grid: Omega elementwise at 1e-12 and the per-column
+    minimum (index, Delta*, Omega*) against the oracle's (reading G11 for near-ties).  A one-q call is split into many short
+    k-chunks; the launch bench.py times (all q in one call, few long chunks) is test_full_size_configs_all_q_launch_parity."""
     import torch
     runs = _golden_runs(cfg)
     if cfg == 5:
@@ -873,7 +878,6 @@ def test_full_size_configs_sampled_parity(fe, cfg, mode):
         with fe.FreeEnergy(w.params, w.N, T) as F:
             F.set_eval_mode(mode)
             for iq in iqs:
-                # the launch configuration bench.py times: the full (h, Delta) grid of the config
                 om = F.omega_grid(w.q[iq:iq + 1], w.h, w.delta)
                 idx, ds, os_ = F.argmin(om, w.delta)
                 torch.cuda.synchronize()
@@ -890,11 +894,45 @@ def test_full_size_configs_sampled_parity(fe, cfg, mode):
                     assert err < RTOL, f"cfg{cfg} {w.name} T={T} col ({iq},{ih}): {err:.3e}"
                     n_exact += check_argmin(ref[None, :], w.delta, idx[ih:ih + 1], ds[ih:ih + 1], os_[ih:ih + 1])
                     n_cols += 1
-    assert n_cols == {3: 12, 4: 32, 5: 12 if mode else 4}[cfg]
+    assert n_cols == {3: 64, 4: 32, 5: 12 if mode else 4}[cfg]
     assert n_exact >= n_cols // 2          # most stored columns have a resolved minimum (index compared bit-exactly)
 
 
-@pytest.mark.parametrize("cfg,sym,ncols", [(4, 3, 32), (3, 1, 12), (5, 1, 12)])
+@pytest.mark.parametrize("mode", [4, 3])
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_configs_all_q_launch_parity(fe, cfg, mode):
+    """The launch bench.py times, against the oracle: ONE fe_omega_grid call over the config's WHOLE q list (mirror symmetry
+    off), in the default early-out mode and in the dense variant, for config 3, config 4 at both temperatures and config 5
+    with seeds 1-3.  With all q in one call the k-sum is cut into few long chunks (config 4: 74 chunks of 14 208 k-points,
+    grid 9472), so the exponent sums and the renormalisation cadence are those of the benchmark, not those of a one-q call.
+    Every stored whole oracle column: Omega elementwise at 1e-12, and the per-column minimum (reading G11)."""
+    import torch
+    n_cols = n_exact = 0
+    for w, T, cols in _golden_runs(cfg):
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            F.set_eval_mode(mode)
+            om = F.omega_grid(w.q, w.h, w.delta)
+            idx, ds, os_ = F.argmin(om, w.delta)
+            torch.cuda.synchronize()
+            info = F.last_launch_info()
+            assert info["mode"] == mode and F.last_symmetry() == 0
+            if cfg == 4:
+                assert info["grid"] == 9472 and info["ksplit"] == 74 and info["rows_per_chunk"] == 14208
+        om, idx, ds, os_ = om.cpu().numpy(), idx.cpu().numpy(), ds.cpu().numpy(), os_.cpu().numpy()
+        assert np.array_equal(idx, np.argmin(om, axis=-1).astype(np.int32)) and np.array_equal(os_, om.min(axis=-1))
+        for c in cols:
+            iq, ih = c["iq"], c["ih"]
+            assert c["id"] == list(range(w.nd)), "golden columns must be whole columns"
+            ref = np.array([float(x) for x in c["omega"]])
+            err = max_rel(om[iq, ih], ref)
+            assert err < RTOL, f"cfg{cfg} {w.name} T={T} mode {mode} col ({iq},{ih}): {err:.3e}"
+            n_exact += check_argmin(ref[None, :], w.delta, idx[iq, ih:ih + 1], ds[iq, ih:ih + 1], os_[iq, ih:ih + 1])
+            n_cols += 1
+    assert n_cols == {3: 64, 4: 32, 5: 12}[cfg]
+    assert n_exact >= n_cols // 2
+
+
+@pytest.mark.parametrize("cfg,sym,ncols", [(4, 3, 32), (3, 1, 64), (5, 1, 12)])
 def test_symmetry_reduced_ksum_full_size_configs(fe, cfg, sym, ncols):
     """Configs 3-5 with fe_set_symmetry (config 4: q on the (1,1) diagonal, k_x <-> k_y, the launch configuration bench.py
     times as `symmetric_variant`; configs 3 and 5: q = (q_x, 0), k_y -> -k_y), all q in one call: the stored whole oracle
