@@ -608,6 +608,8 @@ def main():
         F.enable_slot_counts(True)
         for s in range(len(temps)):
             one_step(args.warmup + s)
+            if F.last_launch_info()["mode"] not in (fe.EVAL_COOP, fe.EVAL_COOP_EO):
+                break                                   # a grid far smaller than a block tile ran on the per-thread kernel: no slots
             c = F.slot_counts()                         # waits for the launch, reads five counters
             tot = c["dense"] + c["a_dominated"] + c["b_dominated"]
             slot_kinds[f"T={temps[(args.warmup + s) % len(temps)]:g}"] = {k: v / tot for k, v in c.items()}

@@ -146,6 +146,14 @@ def config(i, seed=1):
         b = three_band(N=1024, U=1.5, T=0.001, nq=32, nh=64, nd=512, qdir="diag")
         b.name = "B3_fflo_N1024"
         return b
+    if i == 7:     # not in BASELINE.json: config 4's shape on an interior-minimum grid (U = 5: Delta* > 0 on most columns),
+        w = interior_minimum(N=1024, U=5.0, T=0.001, nq=32, nh=64, nd=512)      # to show how data-dependent the early-out is
+        w.T, w.name, w.q = (0.001, 0.01), "X_U5_fflo_N1024", _q_diag(np.linspace(0.0, 0.2 * pi, 32))
+        return w
+    if i == 8:     # not in BASELINE.json: config 4 at a high temperature (wide dominance window: more slots stay dense)
+        w = config(4)
+        w.T, w.name = (0.02,), "cfg4_fflo_N1024_T0.02"
+        return w
     raise ValueError(f"no such config: {i}")
 
 

@@ -74,6 +74,49 @@ def test_bench_rank_mapping_and_gather_world2():
     assert ret[("calls", 0)] == [3, 5, 1] and ret[("calls", 1)] == [2, 5]     # rank 1's shard of a 1-q list is empty
 
 
+def _worker8(rank, world, port, ret):
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import bench
+    from paper_1412_8754_b200 import workloads as W
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = W.config(4)                                    # the headline q list: 32 q over 8 ranks = 4 q per rank
+
+    def evaluate(qs, h, delta):                        # a stub with a recognisable answer per (q, h): no Omega needed here
+        qs = np.asarray(qs).reshape(-1, 2)
+        v = qs[:, :1] * 1000.0 + np.asarray(h)[None, :]
+        return (v * 7).astype(np.int32), v + 0.5, -v
+
+    g = bench.sharded_scan(evaluate, w.q, w.h, w.delta, rank, world, "strong")
+    idx, qs, ntot = bench.rank_q(w.q, rank, world, "strong")
+    few = bench.sharded_scan(evaluate, w.q[:3], w.h, w.delta, rank, world, "strong")      # more ranks than q-values
+    ret[rank] = (idx.tolist(), ntot, g["idx"], g["delta_star"], g["omega_star"], few["omega_star"])
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_bench_rank_mapping_and_gather_world8_config4():
+    """bench.py --gpus 8 on the headline config, host side: 32 q round-robin over 8 ranks (4 each), every rank ends with
+    all 32 x 64 minima in q order; and a 3-q list on 8 ranks (5 empty shards that still take part in the gather)."""
+    from paper_1412_8754_b200 import workloads as W
+    w = W.config(4)
+    mgr = mp.Manager()
+    ret = mgr.dict()
+    mp.spawn(_worker8, args=(8, _free_port(), ret), nprocs=8, join=True)
+    v = w.q[:, :1] * 1000.0 + w.h[None, :]
+    owned = []
+    for r in range(8):
+        idx, ntot, gi, gd, go, few = ret[r]
+        assert idx == list(range(r, 32, 8)) and ntot == 32
+        assert gi.shape == (32, 64) and np.array_equal(gi, (v * 7).astype(np.int32))
+        assert np.array_equal(gd, v + 0.5) and np.array_equal(go, -v)
+        assert few.shape == (3, 64) and np.array_equal(few, -v[:3])
+        owned += idx
+    assert sorted(owned) == list(range(32))             # every q-value has exactly one owner
+
+
 CSV_HEAD = '"ID","Process ID","Process Name","Host Name","Kernel Name","Context","Stream","Block Size","Grid Size","Device","CC","Section Name","Metric Name","Metric Unit","Metric Value"\n'
 
 

@@ -226,6 +226,63 @@ def test_argmin_q_bit_exact_and_vs_oracle(fe, oracle):
             assert abs(val[ih] - rv[ih]) <= 2 * RTOL * scale        # a difference of two Omega values
 
 
+def _check_argmin_q(ref, tol, iq, idd, val):
+    """(iq, id, value) per h against the oracle grid `ref` (condensation energies, ref_id = 0): where the oracle's best and
+    second-best differ by more than 10 tol the index pair must agree, else any pair inside that band is valid (reading G11)."""
+    ce = ref - ref[:, :, :1]
+    n_exact = 0
+    for ih in range(ref.shape[1]):
+        flat = ce[:, ih, :].reshape(-1)
+        best = int(np.argmin(flat))
+        srt = np.sort(flat)
+        if srt[1] - srt[0] > 10 * tol:
+            assert (iq[ih], idd[ih]) == divmod(best, ref.shape[2]), (ih, iq[ih], idd[ih], divmod(best, ref.shape[2]))
+            n_exact += 1
+        else:
+            assert ce[iq[ih], ih, idd[ih]] - flat[best] <= 10 * tol
+        assert abs(val[ih] - flat[best]) <= 2 * tol
+    return n_exact
+
+
+@pytest.mark.parametrize("model", [2, 3])
+def test_per_band_minimisation_against_oracle(fe, oracle, model):
+    """PAPER.md:125 / :92: every band eps minimised on its own over (q, Delta), "(q_eps, Delta_eps)": one handle per
+    band_mask bit with the condensation term counted once, fe_omega_grid -> fe_argmin_q(ref_id = 0), against the oracle's
+    grid for the same mask.  A single band's Omega can be a small difference of large sums (S - P), so the tolerance is
+    relative to the oracle's own summed magnitude (1e-13 of it), as in the randomised tests with a band mask."""
+    from paper_1412_8754_b200 import sweep
+    w = W.interior_minimum(N=48, U=5.0, T=0.004, nq=5, nh=6, nd=40) if model == 2 else W.three_band(N=40, nq=4, nh=6, nd=30)
+    T = w.T[0]
+    got = sweep.per_band_minima(w.params, w.N, T, w.q, w.h, w.delta)
+    assert len(got) == model
+    n_exact = 0
+    for e, g in enumerate(got):
+        pe = dict(w.params, band_mask=1 << e, cond_mult=1.0)
+        ref = oracle.omega_grid(pe, w.N, T, w.q, w.h, w.delta)
+        tol = 1e-13 * float(oracle.omega_grid_magnitude(pe, w.N, T, w.q, w.h, w.delta).max())
+        n_exact += _check_argmin_q(ref, tol, g["iq"], g["id"], g["value"])
+        rq, rd, rv = oracle.argmin_q(ref, ref_id=0)
+        assert np.all(np.abs(g["value"] - rv) <= 2 * tol)
+    assert n_exact >= 4            # fields with a superconducting band minimum have a unique (q, Delta); at Delta = 0 every q ties
+
+
+def test_h_T_sweep_phase_diagram_against_oracle(fe, oracle):
+    """The (h, T) loop of PAPER.md:125 on a 3 x 4 (T, h) grid: sweep.phase_diagram (one handle, fe_set_temperature per T,
+    fe_omega_grid -> fe_argmin_q) against the oracle evaluated per temperature."""
+    from paper_1412_8754_b200 import sweep
+    w = W.interior_minimum(N=48, U=5.0, T=0.002, nq=5, nh=4, nd=40)
+    Ts = (0.002, 0.01, 0.03)
+    pd = sweep.phase_diagram(w.params, w.N, w.q, w.h, w.delta, Ts, ref_id=0)
+    assert pd["iq"].shape == (3, 4) and pd["q_star"].shape == (3, 4, 2) and pd["delta_star"].shape == (3, 4)
+    n_exact = 0
+    for it, T in enumerate(Ts):
+        ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+        n_exact += _check_argmin_q(ref, RTOL * float(np.abs(ref).max()), pd["iq"][it], pd["id"][it], pd["value"][it])
+        assert np.array_equal(pd["delta_star"][it], w.delta[pd["id"][it]]) and np.array_equal(pd["q_star"][it], w.q[pd["iq"][it]])
+    assert n_exact >= 4            # normal-state columns (Delta* = 0) tie over q by construction: condensation energy 0
+    assert not np.array_equal(pd["id"][0], pd["id"][2])        # the order parameter melts between T = 0.002 and T = 0.03
+
+
 # ---- static Cooper-pair susceptibility (SURVEY.md 8f-4, Appendix C) ----
 @pytest.mark.parametrize("model", [1, 2, 3])
 def test_pair_susceptibility_parity(fe, oracle, model):
@@ -669,6 +726,46 @@ def test_slot_counters_and_moment_series(fe, oracle):
                 assert c["a_dominated"] > 0.5 * c["dense"] and 0 < c["a_series"] <= c["a_dominated"]
                 if w.name == "big_delta":
                     assert c["a_series"] < c["a_dominated"]          # some dominated slots have eps > 1/16: list path
+
+
+def test_early_out_bias_at_the_dominance_threshold(fe, oracle):
+    """The early-out replaces T ln Z by R_j on a slot whose 2cosh(R_j/T) leads 2cosh(|d_i|/T) by 2^44 (kDomGap) over the
+    block tile; what it drops, T ln(1 + B/A), is one-signed and below 5.1e-15 R_j per term (include/fe.h, FE_EVAL_COOP_EO).
+    Worst case for that bound: a narrow filled band (s = -1 +- 0.02, |d| < 0.003) at T = 1 / (44 ln 2), so that R / (T ln 2) runs
+    over [43.1, 44.9] and EVERY slot sits within a binade of the threshold -- about half of them just above it (dominated,
+    A / B between 2^43 and 2^44), half just below (dense).  Early-out minus
+    dense is then a systematic, positive shift of Omega; it must stay below 5.1e-15 x (sum of R over the dominated slots),
+    and both must still match the oracle."""
+    import torch
+    t, mu = 0.005, 1.0            # filled band: s = E - mu ~ -1, so Omega ~ -2 N^2 is well conditioned
+    T = 1.0 / (44.0 * np.log(2.0))
+    params = W.model_params(model=W.MODEL_ONE_BAND, form_factor=W.FORM_S, t=(t,), mu=mu, U=2.0)
+    w = W.Workload("dom_threshold", params, 64, (T,), np.array([[0.1, 0.05]]), np.linspace(0.0, 0.002, 64),
+                   np.linspace(0.0, 0.01, 128))
+    res = {}
+    for mode in (fe.EVAL_COOP_EO, fe.EVAL_COOP):
+        with fe.FreeEnergy(w.params, w.N, T) as F:
+            F.set_eval_mode(mode)
+            F.set_coop_shape(1)                         # 64 x 128 block tile: the whole (h, Delta) grid is ONE tile
+            F.enable_slot_counts(True)
+            om = F.omega_grid(w.q, w.h, w.delta)
+            c = F.slot_counts()
+            torch.cuda.synchronize()
+            assert (F.last_launch_info()["th"], F.last_launch_info()["td"]) == (64, 128)
+        res[mode] = (om.cpu().numpy(), c)
+    (eo, c_eo), (dense, c_dense) = res[fe.EVAL_COOP_EO], res[fe.EVAL_COOP]
+    nslots = w.N * w.N
+    assert c_dense["a_dominated"] == 0 and c_eo["dense"] + c_eo["a_dominated"] + c_eo["b_dominated"] == nslots
+    assert 0.2 * nslots < c_eo["a_dominated"] < 0.95 * nslots and c_eo["dense"] > 0.05 * nslots, c_eo   # threshold cuts through the band
+    ref = oracle.omega_grid(w.params, w.N, T, w.q, w.h, w.delta)
+    assert max_rel(eo, ref) < RTOL and max_rel(dense, ref) < RTOL
+    diff = eo - dense                                   # P is underestimated, Omega = S - P + ... overestimated: diff >= 0
+    ulp = np.spacing(np.abs(dense).max())
+    r_max = abs(mu) + 4 * t + float(np.abs(w.delta).max())
+    bound = 5.1e-15 * c_eo["a_dominated"] * r_max
+    assert diff.max() <= bound + 4 * ulp, (diff.max(), bound, ulp)
+    assert diff.min() >= -4 * ulp, (diff.min(), ulp)
+    assert diff.mean() > 0.0, "the neglected part is one-signed: on this grid it must show as a positive shift"
 
 
 def test_factored_extreme_spreads(fe, oracle):
