@@ -276,6 +276,18 @@ def rank_q(w_q, rank, world, scaling):
     raise ValueError(scaling)
 
 
+def job_reduce(x, op, world, device="cuda", group=None):
+    """One number per rank -> the job's number on every rank: op = "sum" (units all ranks processed in a step) or "max"
+    (the slowest rank's time: what the whole job takes).  The only collectives bench.py issues besides the gather of the
+    minima; world == 1 returns x unchanged.  `device` is "cuda" under NCCL, "cpu" in the gloo test of this function."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op={"sum": dist.ReduceOp.SUM, "max": dist.ReduceOp.MAX}[op], group=group)
+    return float(t.item())
+
+
 def sharded_scan(evaluate, w_q, h, delta, rank, world, scaling, group=None):
     """One multi-GPU pass: this rank evaluates its q-values with `evaluate(q, h, delta) -> (idx, delta*, omega*)`
     (FreeEnergy.scan_host on a GPU; a stub in the CPU test) and the minima of all ranks are gathered in column order."""
@@ -370,6 +382,7 @@ def run_chi(args):
     host = torch.empty((w.nq, nb, nb), dtype=torch.float64).pin_memory()
     hq = torch.from_numpy(w.q.copy()).pin_memory().numpy()
     e2e_steps = max(5, min(args.steps, 10))
+    e2e_steps += (-e2e_steps) % len(temps)           # whole cycles of the alternating temperatures: the same mix as an even K
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         F.pair_susceptibility(hq, hz, out=chi, stream=stream)
@@ -565,10 +578,7 @@ def main():
 
     evals_rank_step = w.N * w.N * nq_step * w.nh * w.nd
     # units all ranks process per step (strong: the job's q list once; weak: once per rank)
-    t_e = torch.tensor([float(evals_rank_step)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_e, op=dist.ReduceOp.SUM)
-    evals_job_step = float(t_e.item())
+    evals_job_step = job_reduce(evals_rank_step, "sum", world)
     for s in range(args.warmup):
         one_step(s)
     barrier()
@@ -617,10 +627,7 @@ def main():
     idx_check = int(res[0].sum().item()) if res is not None else 0      # device->host read of the step's result
 
     total_ms = sum(step_ms)
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
+    total_ms_max = job_reduce(total_ms, "max", world)
     value = evals_job_step * args.steps / (total_ms_max * 1e-3)
 
     # ---- the dense variant of the same kernel (every pair multiplied out), timed beside the early-out default:
@@ -712,11 +719,9 @@ def main():
         F.set_temperature(temps[s % len(temps)])
         gathered = sharded_scan(scan_host_eval, w.q, hh, hd, rank, world, args.scaling)
     torch.cuda.synchronize()
-    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_seconds = job_reduce(time.perf_counter() - t0, "max", world)
     evals_job_scan = w.N * w.N * ncols_job * w.nh * w.nd
-    e2e_value = evals_job_scan * e2e_steps / float(te.item())
+    e2e_value = evals_job_scan * e2e_steps / e2e_seconds
     assert gathered["idx"].shape == (ncols_job, w.nh)
     h2d = 8 * (2 * nq_rank + w.nh + 2 * w.nd)           # q, h, Delta^2 lists + Delta list for the argmin
     d2h = 8 * nq_rank * w.nh * w.nd + nq_rank * w.nh * (4 + 8 + 8)

@@ -45,6 +45,10 @@ def _worker(rank, world, port, ret):
     g1 = bench.sharded_scan(evaluate, w.q[:1], w.h, w.delta, rank, world, "strong")
     ret[("one", rank)] = g1["idx"]
     ret[("calls", rank)] = calls
+    # the two reductions of bench.py's N > 1 path (units per step summed, times maximised), on CPU tensors over gloo
+    ret[("reduce", rank)] = (bench.job_reduce(3.0 + rank, "sum", world, device="cpu"),
+                             bench.job_reduce(10.0 * (rank + 1), "max", world, device="cpu"),
+                             bench.job_reduce(5.0, "max", 1, device="cpu"))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -72,6 +76,7 @@ def test_bench_rank_mapping_and_gather_world2():
         assert ntot == 10 and np.array_equal(gi, np.vstack([ref[0]] * 2)) and np.array_equal(go, np.vstack([ref[2]] * 2))
         assert np.array_equal(ret[("one", r)], ref[0][:1])
     assert ret[("calls", 0)] == [3, 5, 1] and ret[("calls", 1)] == [2, 5]     # rank 1's shard of a 1-q list is empty
+    assert ret[("reduce", 0)] == (7.0, 20.0, 5.0) and ret[("reduce", 1)] == (7.0, 20.0, 5.0)
 
 
 def _worker8(rank, world, port, ret):

@@ -181,3 +181,29 @@ def test_three_band_symmetries_and_band_mask(oracle):
     assert rel(a[1], c[1]) < 1e-13                                     # q -> -q
     parts = [oracle.omega_column(dict(THREE, band_mask=1 << e, cond_mult=1.0), N, T, (0.3, 0.1), 0.02, d) for e in range(3)]
     assert np.max(np.abs(sum(parts) - a) / np.abs(a)) < 1e-13          # Omega = sum_eps Omega_eps
+
+
+def test_three_band_matrix_lattice_symmetries(oracle):
+    """A pin of feo_three_band_matrix that does not retype B.1-B.6: what the square lattice and the orbitals fix.
+    The xz / yz orbitals swap under k_x <-> k_y and xy maps to itself, so T(k_y, k_x) = P T(k_x, k_y) P^T with P the swap
+    of orbitals 1 and 2; under k_x -> -k_x the xz orbital changes sign, T(-k_x, k_y) = D T(k_x, k_y)* D ... in every case
+    the SPECTRUM is unchanged.  A slip in one matrix element (t1 and t2 exchanged in one diagonal entry, a sign in the
+    t11 term, sin for cos in an off-diagonal entry, a wrong k component) breaks at least one of: Hermiticity,
+    2 pi periodicity, the three mirror invariances of the eigenvalues, the orbital-swap identity of the matrix itself,
+    inversion T(-k) = T(k)* (time reversal for spinless hoppings)."""
+    rng = np.random.default_rng(5)
+    P = np.array([[0, 1, 0], [1, 0, 0], [0, 0, 1]], dtype=float)
+    for _ in range(200):
+        kx, ky = rng.uniform(-PI, PI, size=2)
+        M = oracle.three_band_matrix(THREE, kx, ky)
+        assert np.abs(M - M.conj().T).max() < 1e-15
+        assert np.abs(M - oracle.three_band_matrix(THREE, kx + 2 * PI, ky - 2 * PI)).max() < 1e-13
+        ev = np.linalg.eigvalsh(M)
+        for k2 in ((ky, kx), (-kx, ky), (kx, -ky), (-kx, -ky)):
+            assert np.abs(np.linalg.eigvalsh(oracle.three_band_matrix(THREE, *k2)) - ev).max() < 1e-13
+        # the matrix identities behind two of them
+        assert np.abs(oracle.three_band_matrix(THREE, ky, kx) - P @ M @ P.T).max() < 1e-14
+        assert np.abs(oracle.three_band_matrix(THREE, -kx, -ky) - M.conj()).max() < 1e-14
+    # and the band energies the oracle's Omega uses are those eigenvalues, ascending
+    kx, ky = 0.3, -1.1
+    assert np.abs(oracle.band_energies(THREE, kx, ky) - np.linalg.eigvalsh(oracle.three_band_matrix(THREE, kx, ky))).max() < 1e-13

@@ -90,6 +90,31 @@ def test_static_entry_point_one_band_and_the_documented_example_size(fe):
     assert max_rel(out.cpu().numpy(), handle_path(fe, w, w.T[0])) < RTOL
 
 
+def test_static_entry_point_leaves_free_device_memory_unchanged(fe):
+    """What "allocates nothing" means for the caller, observed from outside: after the first call on the device (set-up,
+    and the driver loading the kernels), the free device memory reported by the driver (cudaMemGetInfo, i.e. including
+    everything outside PyTorch's pool) is the same before and after further calls -- also calls that use more of the fixed
+    array than any earlier one.  The handle path, for contrast, takes memory for its scratch."""
+    import torch
+    small = W.ragged(seed=3, N=33, nq=2, nh=3, nd=17)
+    big = W.interior_minimum(N=512, U=5.0, T=0.004, nq=2, nh=32, nd=256)     # 2 column groups x 16384 outputs of partial sums
+    out_small = torch.empty((small.nq, small.nh, small.nd), dtype=torch.float64, device="cuda")
+    out_big = torch.empty((big.nq, big.nh, big.nd), dtype=torch.float64, device="cuda")       # outputs are the caller's: made first
+    fe.omega_grid_static(small.params, small.N, small.T[0], small.q, small.h, small.delta, out_small)    # set-up happens here at the latest
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(2):
+        fe.omega_grid_static(big.params, big.N, big.T[0], big.q, big.h, big.delta, out_big)
+        fe.omega_grid_static(small.params, small.N, small.T[0], small.q, small.h, small.delta, out_small)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0, "fe_omega_grid_static changed the device's free memory"
+    assert max_rel(out_big.cpu().numpy(), handle_path(fe, big, big.T[0])) < RTOL
+    with fe.FreeEnergy(big.params, big.N, big.T[0]) as F:                       # contrast: the handle path allocates scratch
+        F.omega_grid(big.q, big.h, big.delta, out=out_big)
+        torch.cuda.synchronize()
+        assert torch.cuda.mem_get_info()[0] < free0
+
+
 def test_static_entry_point_refuses_what_does_not_fit(fe):
     import torch
     L = fe.lib()
