@@ -61,7 +61,7 @@ struct CoopParams {
   const double* etab;                  // NB == 3 only: [1 + nq][3][N*N] band tables, y = 0: E(k), 1 + iq: E(k - q)
   double* partial;                     // [ksplit][nq*nh*nd]
   unsigned long long* kind_counts;     // NULL, or 5 device counters {dense, A-dominated (list), B-dominated, padding, A-dominated
-                                       // (moment series)} slots, summed over all blocks of the launch (fe_enable_timing)
+                                       // (moment series)} slots, summed over all blocks of the launch (fe_enable_slot_counts)
 };
 
 struct __align__(16) CoopHdr {         // one per (k, band) slot
