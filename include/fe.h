@@ -222,8 +222,10 @@ int fe_scan_host(fe_handle* h,
  * quantity, its value and the limit, and touches nothing):
  *   2 nq + nh + nd <= FE_STATIC_MAX_LIST,  nq N <= FE_STATIC_MAX_TRIG,  nq nh nd <= FE_STATIC_MAX_OUT,
  *   ceil(N / 256) nq nh nd <= FE_STATIC_MAX_PARTIAL.   Example that fits: N = 1024, 1 q, 16 h, 512 Delta.
- * It evaluates every term directly (the FE_EVAL_DIRECT formulation of fe_debug.h, the slowest and most literal one), which
- * is adequate at these sizes; results agree with fe_omega_grid to rounding (~1e-14 relative) and are deterministic.
+ * It evaluates every term directly (the FE_EVAL_DIRECT formulation of fe_debug.h, the slowest and most literal one):
+ * the example above takes 57 ms on a B200 where fe_omega_grid's default kernel takes 2.5 ms, so this is the path for
+ * callers who cannot allocate, not a fast path.  Results agree with fe_omega_grid to rounding (5e-15 relative measured
+ * on that example) and are deterministic.
  *
  * First call on a device: it looks up the device address of the array (cudaGetSymbolAddress, once per device, with that
  * device current) and copies the math tables into it with a host-synchronous cudaMemcpy.  Make that first call during
